@@ -1,0 +1,173 @@
+"""Pins for the Euler oracle (BASELINE.json config 4; MUSCL/minmod/Rusanov midpoint, readings E1-E5)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+G = wl.EULER_GAMMA
+
+
+def _prim(U, gamma=G):
+    rho, m, E = U
+    u = m / rho
+    return rho, u, (gamma - 1) * (E - 0.5 * m * u)
+
+
+def test_uniform_state_is_fixed_point_exactly():
+    U0 = wl.euler_conserved(np.full(32, 0.9), np.full(32, 0.4), np.full(32, 1.7))
+    U = oracle.euler(U0, 20, G, 1 / 32, 0.2 / 32)
+    assert np.array_equal(U, U0)
+
+
+def test_conservation_and_positivity_sod():
+    w = wl.euler_config4(1024)
+    U0 = w.initial(np.float64)
+    U = oracle.euler(U0, 2000, w.gamma, w.dx, w.dt)          # raises if rho or p go non-positive
+    s0, s1 = U0.sum(axis=1), U.sum(axis=1)
+    assert abs(s1[0] - s0[0]) < 1e-13 * abs(s0[0])
+    assert abs(s1[2] - s0[2]) < 1e-13 * abs(s0[2])
+    assert abs(s1[1]) < 1e-11                                   # total momentum stays 0 (mirror symmetry)
+    rho, u, p = _prim(U)
+    assert rho.min() > 0 and p.min() > 0
+    assert np.abs(u).max() > 0.5                                # waves really moved
+
+
+def test_conservation_noise_state():
+    w = wl.euler_noise(512, seed=2)
+    U0 = w.initial(np.float64)
+    U = oracle.euler(U0, 300, w.gamma, w.dx, w.dt)
+    for k in range(3):
+        assert abs(U[k].sum() - U0[k].sum()) < 1e-12 * np.abs(U0[k]).sum()
+    assert np.max(np.abs(U - U0)) > 0.05
+
+
+def test_mirror_symmetry():
+    """Cell-centred grid, high state on [1/4, 3/4): rho, E even and m odd about x = 1/2 (reading E3)."""
+    w = wl.euler_config4(512)
+    U = oracle.euler(w.initial(np.float64), 600, w.gamma, w.dx, w.dt)
+    assert np.max(np.abs(U[0] - U[0][::-1])) < 1e-12
+    assert np.max(np.abs(U[2] - U[2][::-1])) < 1e-12
+    assert np.max(np.abs(U[1] + U[1][::-1])) < 1e-12
+
+
+def _sod_star(gamma=G, L=(1.0, 0.0, 1.0), R=(0.125, 0.0, 0.1)):
+    """Exact Riemann solver for the star region: Newton iteration on the pressure function."""
+    rl, ul, pl = L
+    rr, ur, pr = R
+    cl, cr = np.sqrt(gamma * pl / rl), np.sqrt(gamma * pr / rr)
+
+    def fk(p, rk, pk, ck):
+        if p > pk:      # shock
+            A, B = 2 / ((gamma + 1) * rk), (gamma - 1) / (gamma + 1) * pk
+            f = (p - pk) * np.sqrt(A / (p + B))
+            df = np.sqrt(A / (p + B)) * (1 - (p - pk) / (2 * (B + p)))
+        else:           # rarefaction
+            f = 2 * ck / (gamma - 1) * ((p / pk) ** ((gamma - 1) / (2 * gamma)) - 1)
+            df = 1 / (rk * ck) * (p / pk) ** (-(gamma + 1) / (2 * gamma))
+        return f, df
+
+    p = 0.5 * (pl + pr)
+    for _ in range(50):
+        fl, dfl = fk(p, rl, pl, cl)
+        fr, dfr = fk(p, rr, pr, cr)
+        p_new = p - (fl + fr + ur - ul) / (dfl + dfr)
+        if abs(p_new - p) < 1e-14:
+            p = p_new
+            break
+        p = p_new
+    u = 0.5 * (ul + ur) + 0.5 * (fk(p, rr, pr, cr)[0] - fk(p, rl, pl, cl)[0])
+    rsl = rl * (p / pl) ** (1 / gamma)                                             # behind the rarefaction
+    rsr = rr * ((p / pr + (gamma - 1) / (gamma + 1)) / ((gamma - 1) / (gamma + 1) * p / pr + 1))  # behind the shock
+    return p, u, rsl, rsr
+
+
+def test_exact_riemann_solver_reproduces_textbook_sod_values():
+    gold = dict(line.split()[:2] for line in open(os.path.join(GOLD, "sod_star_state.txt")) if not line.startswith("#"))
+    p, u, rsl, rsr = _sod_star()
+    assert p == pytest.approx(float(gold["p_star"]), abs=1e-5)
+    assert u == pytest.approx(float(gold["u_star"]), abs=1e-5)
+    assert rsl == pytest.approx(float(gold["rho_star_L"]), abs=1e-5)
+    assert rsr == pytest.approx(float(gold["rho_star_R"]), abs=1e-5)
+
+
+def test_sod_star_states_before_the_mirrored_waves_meet():
+    """At t = 0.1 (< 0.14) each half of the mirrored tube is the textbook Sod solution."""
+    nx = 4096
+    w = wl.euler_config4(nx)
+    n = int(round(0.1 / w.dt))
+    t = n * w.dt
+    U = oracle.euler(w.initial(np.float64), n, w.gamma, w.dx, w.dt)
+    rho, u, p = _prim(U)
+    ps, us, rsl, rsr = _sod_star()
+    x = (np.arange(nx) + 0.5) / nx
+    cs = np.sqrt(G * ps / rsl)
+    tail, contact = 0.75 + (us - cs) * t, 0.75 + us * t
+    shock = 0.75 + t * np.sqrt(G * 0.1 / 0.125) * np.sqrt((G + 1) / (2 * G) * ps / 0.1 + (G - 1) / (2 * G))
+    i1 = np.argmin(np.abs(x - 0.5 * (tail + contact)))
+    i2 = np.argmin(np.abs(x - 0.5 * (contact + shock)))
+    assert rho[i1] == pytest.approx(rsl, abs=1e-3) and u[i1] == pytest.approx(us, abs=1e-3) and p[i1] == pytest.approx(ps, abs=1e-3)
+    assert rho[i2] == pytest.approx(rsr, abs=1e-3) and u[i2] == pytest.approx(us, abs=1e-3) and p[i2] == pytest.approx(ps, abs=1e-3)
+    # mirrored copy at x = 0.25 moves the other way
+    j1 = nx - 1 - i1
+    assert rho[j1] == pytest.approx(rsl, abs=1e-3) and u[j1] == pytest.approx(-us, abs=1e-3)
+    # undisturbed states away from the waves
+    assert rho[nx // 2] == 1.0 and rho[0] == 0.125
+
+
+def _euler_numpy_step(U, gamma, lam):
+    """Independent second evaluation: vectorised np.roll form of the textbook formulas (no fma order)."""
+
+    def minmod(a, b):
+        return np.where(a * b > 0, np.where(np.abs(a) < np.abs(b), a, b), 0.0)
+
+    def flux(W):
+        rho, m, E = W
+        u = m / rho
+        p = (gamma - 1) * (E - 0.5 * m * u)
+        return np.stack([m, m * u + p, (E + p) * u]), np.abs(u) + np.sqrt(gamma * p / rho)
+
+    def rhs(W):
+        sig = minmod(W - np.roll(W, 1, axis=1), np.roll(W, -1, axis=1) - W)
+        WL = W + 0.5 * sig
+        WR = np.roll(W - 0.5 * sig, -1, axis=1)
+        fL, sL = flux(WL)
+        fR, sR = flux(WR)
+        F = 0.5 * (fL + fR) - 0.5 * np.maximum(sL, sR) * (WR - WL)      # F_{i+1/2}
+        return F - np.roll(F, 1, axis=1)
+
+    Us = U - 0.5 * lam * rhs(U)
+    return U - lam * rhs(Us)
+
+
+@pytest.mark.parametrize("nx,n", [(8, 3), (64, 40)])
+def test_tiny_grid_against_independent_evaluation(nx, n):
+    rng = np.random.default_rng(nx)
+    U0 = wl.euler_conserved(1 + 0.4 * rng.uniform(-1, 1, nx), 0.5 * rng.uniform(-1, 1, nx), 1 + 0.4 * rng.uniform(-1, 1, nx))
+    dx = 1.0 / nx
+    dt = 0.2 * dx
+    V = U0.copy()
+    for _ in range(n):
+        V = _euler_numpy_step(V, G, dt / dx)
+    U = oracle.euler(U0, n, G, dx, dt)
+    assert np.max(np.abs(U - V)) < 1e-13 * np.max(np.abs(V)) * n
+    assert np.max(np.abs(U - U0)) > 1e-3
+
+
+def test_shift_equivariance_bitwise_and_fp32_runs_in_fp32():
+    w = wl.euler_noise(128, seed=9)
+    U0 = w.initial(np.float32)
+    a = oracle.euler(np.roll(U0, 45, axis=1), 30, w.gamma, w.dx, w.dt)
+    b = np.roll(oracle.euler(U0, 30, w.gamma, w.dx, w.dt), 45, axis=1)
+    assert a.dtype == np.float32 and np.array_equal(a, b)
+    d = oracle.euler(w.initial(np.float64), 30, w.gamma, w.dx, w.dt)
+    assert 0 < np.max(np.abs(np.roll(d, 45, axis=1) - b)) < 1e-4
+
+
+def test_positivity_flag_raises():
+    w = wl.euler_config4(256)
+    with pytest.raises(FloatingPointError):
+        oracle.euler(w.initial(np.float64), 200, w.gamma, w.dx, 4.0 * w.dt)   # CFL 2: must break
