@@ -1,0 +1,148 @@
+/* swept1d.h -- C ABI of the B200-native swept time-space decomposition library (libswept1d.so).
+ *
+ * Method: Magee & Niemeyer, "An initial investigation of the performance of GPU-based swept
+ * time-space decomposition" (arXiv 1612.02495), cited below as PAPER.md:<line>.  The library
+ * advances an explicit 1-D scheme on a periodic grid of nx points either
+ *   - by the swept rule: every tile of W points advances through an
+ *     upright triangle, then diamonds on tiles shifted by W/2, then a closing inverted triangle,
+ *     touching global memory once per W/(2h) sub-timesteps, or
+ *   - by the classic decomposition (Fig. 6): one kernel per sub-timestep.
+ * Both evaluate the same device stencil functions, so their results are bit-identical.
+ *
+ * Conventions for every entry point
+ *   - All pointers named d_* are DEVICE pointers, h_* are HOST pointers; sizes are element counts.
+ *   - Field layout: [ncomp][nx] contiguous, structure of arrays (Euler: rho row, m = rho*u row,
+ *     E row; heat and KS: one row), dtype as given at creation, base address 16-byte aligned.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     swept_run / naive_run only ENQUEUE work on that stream: they never synchronise and never
+ *     allocate.  The field holds the solution at time +nsteps*dt when the stream reaches the end
+ *     of the enqueued work.
+ *   - Return value: 0 on success, negative on error (SWEPT_EINVAL / ENOMEM / ECUDA); the message is
+ *     available from swept_last_error() (thread-local).  Nothing is printed, nothing aborts.
+ *     Numerical blow-up is not an error: values become Inf/NaN exactly as the classic path's would.
+ *   - No CPU fallback exists: without a CUDA device every compute call fails with SWEPT_ECUDA.
+ */
+#ifndef SWEPT1D_H
+#define SWEPT1D_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swept_ctx *swept_handle_t; /* opaque; owned by the library */
+
+/* problem -- the per-problem stencil device functions (radius h, stages S, fields ncomp):
+ *   SWEPT_HEAT   FTCS, Eq. (2) PAPER.md:54                                   h=1 S=1 ncomp=1
+ *   SWEPT_KS     Kuramoto-Sivashinsky, Eq. (4),(15),(16) PAPER.md:64,291,295 h=2 S=2 ncomp=1
+ *   SWEPT_EULER  MUSCL/minmod/Rusanov midpoint (BASELINE.json config 4)      h=2 S=2 ncomp=3   */
+enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2 };
+/* dtype -- the paper's compile-time REAL as a run-time choice */
+enum { SWEPT_F32 = 0, SWEPT_F64 = 1 };
+enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_ENOMEM = -2, SWEPT_ECUDA = -3 };
+
+/* Which swept kernels swept_run uses (SWEPT_OPT_KERNEL):
+ *   SWEPT_KERNEL_SMEM  the paper's design (Fig. 5): one block per tile, one
+ *                      thread per point, two-row shared-memory matrix, a block barrier per tier.
+ *   SWEPT_KERNEL_WAVE  B200 design: one lane group per tile, tile values resident in registers,
+ *                      tiers evaluated as a lane-skewed wavefront over the diamond's characteristic
+ *                      lattice, halos by warp shuffle (generalises PAPER.md:183).  Default.      */
+enum { SWEPT_KERNEL_SMEM = 0, SWEPT_KERNEL_WAVE = 1 };
+
+/* swept_set_option keys */
+enum {
+    SWEPT_OPT_KERNEL = 0,         /* SWEPT_KERNEL_*                                              */
+    SWEPT_OPT_NAIVE_GRAPH = 1,    /* 1: naive_run replays a CUDA graph of its launches (default 0:
+                                     plain launches = the paper's classic program)               */
+    SWEPT_OPT_BLOCKS_PER_SM = 2,  /* cap on resident blocks per SM for the swept kernels, 0 = none */
+    SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
+    SWEPT_OPT_SWEPT_GRAPH = 4     /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
+};
+
+typedef struct {
+    int dtype;          /* SWEPT_F32 | SWEPT_F64                                               */
+    double alpha;       /* heat: thermal diffusivity (Fo = alpha dt / dx^2)       */
+    double gamma;       /* Euler: ratio of specific heats                                      */
+    int max_tile_width; /* upper bound for the tuner's tile-width sweep, 0 = library default   */
+} swept_params_t;
+
+typedef struct {
+    int problem, dtype, radius, stages, ncomp;
+    int64_t nx;
+    int64_t workspace_bytes;     /* device workspace owned by the handle (row R1 / classic's 2nd buffer) */
+    int tuned_tile_width;        /* 0 until swept_tune ran                                      */
+    int64_t launches_last_call;  /* kernels the last swept_run / naive_run enqueued              */
+    int64_t launches_total;      /* kernels enqueued through this handle since creation          */
+    int sm_count;                /* multiprocessors of the device the handle lives on            */
+    int max_smem_per_block;      /* opt-in shared-memory limit per block (bytes)                 */
+} swept_info_t;
+
+/* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's
+ * statement of the problem: PAPER.md:48-66).  nx must be a power of two >= 8 (periodic neighbour
+ * is `& (nx-1)`).  Computes the scheme constants once on the host in double (Fo,
+ * 1-2Fo; 0.25/dx, 1/dx^2, 1/dx^4, dt, dt/2; gamma, gamma-1, dt/dx, dt/2dx -- stored reciprocals
+ * instead of divisions), allocates ncomp*nx elements of device workspace on the
+ * current device, and returns the handle in *out.  `p` may be NULL (= f64, alpha 1, gamma 1.4).
+ * Errors: SWEPT_EINVAL (bad problem/dtype/nx, non-finite or non-positive dx/dt, NULL out),
+ * SWEPT_ENOMEM / SWEPT_ECUDA (allocation or device errors). */
+int swept_create(swept_handle_t *out, int problem, int64_t nx, double dx, double dt, const swept_params_t *p);
+
+/* Advance the field at d_u by nsteps full timesteps IN PLACE with the swept rule:
+ * with L = tile_width/(2h) tiers per half-cycle (L/S timesteps), q = nsteps div (L/S) half-cycles
+ * are run as 1 upright triangle (Fig. 5) + (q-1) diamonds on tiles shifted by W/2 each
+ * launch + 1 closing inverted triangle; the nsteps mod (L/S) remaining
+ * timesteps are run first on narrower tiles / the classic kernel (the paper can only output every
+ * n-th step; reading S3).  Edges are exchanged through d_u itself (even
+ * tiers) and the handle's workspace (odd tiers) -- the paper's left/right arrays.
+ * tile_width: power of two, >= 4h, <= nx, nx % tile_width == 0, L even; 0 = the tuned width (or the
+ * library default if swept_tune has not run).  Result is bit-identical to naive_run.
+ * d_u: device, [ncomp][nx], caller-owned.  Errors: SWEPT_EINVAL (NULL, nsteps < 0, illegal width
+ * or a width whose tile does not fit the chosen kernel), SWEPT_ECUDA (launch error). */
+int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void *cuda_stream);
+
+/* Advance the field by nsteps timesteps with the classic decomposition (Fig. 6): one
+ * kernel per sub-timestep over all nx points, neighbours through `& (nx-1)`, global memory in and
+ * out (heat ping-pongs d_u and the workspace; two-stage schemes write the predictor to the
+ * workspace and accumulate the final stage onto d_u, Fig. 6 `+=`).  Same argument rules as swept_run. */
+int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
+
+/* The paper's best-node-size sweep: time swept_run on d_u_scratch (device,
+ * [ncomp][nx], contents destroyed) for every legal tile width (and kernel launch shape) up to
+ * max_tile_width with at most blocks_per_sm_cap resident blocks per SM (0 = no cap), keep the
+ * fastest in the handle and return it in *best_tile_width (may be NULL).  SYNCHRONISES the stream. */
+int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream);
+
+/* End-to-end convenience used for the `e2e` measurement: copy h_u (HOST, [ncomp][nx], ideally
+ * pinned) to an internal device buffer, swept_run (use_swept != 0) or naive_run on it, copy the
+ * result back into h_u, and synchronise the stream. */
+int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int tile_width, int use_swept, void *cuda_stream);
+
+/* Set a SWEPT_OPT_* option.  SWEPT_EINVAL for unknown keys / values. */
+int swept_set_option(swept_handle_t h, int key, int value);
+
+/* Fill *info (caller-owned). */
+int swept_get_info(swept_handle_t h, swept_info_t *info);
+
+/* 1 if tile_width is legal for this handle and the selected kernel, else 0 (reason in swept_last_error). */
+int swept_tile_width_ok(swept_handle_t h, int tile_width);
+
+/* Measure the plain-ALU peak the swept kernels are bound by: a dependent-free FMA chain of the
+ * given dtype on every SM; returns warp-level FP instructions x 32 lanes per second (thread-level
+ * FP instr/s) in *instr_per_s and the elapsed milliseconds of the timed launch in *ms (may be
+ * NULL).  SYNCHRONISES.  Used by bench.py for the "alu" roofline denominator. */
+int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms, void *cuda_stream);
+
+/* Free the workspace and the handle.  The caller must have synchronised every stream it used. */
+int swept_destroy(swept_handle_t h);
+
+/* Message of the last error on this thread ("" if none).  Never NULL. */
+const char *swept_last_error(void);
+
+/* Library version string (static storage). */
+const char *swept_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWEPT1D_H */

@@ -1,0 +1,212 @@
+"""paper_1612_02495_b200 -- B200-native swept time-space decomposition for explicit 1-D PDE time stepping.
+
+Thin ctypes binding of the C ABI in include/swept1d.h (libswept1d.so, hand-written CUDA for sm_100a).
+Argument marshalling only: every step of the hot path -- the upright-triangle, diamond and closing
+inverted-triangle kernels (Fig. 5), the edge-exchange staircases, the
+classic one-kernel-per-sub-timestep path (Fig. 6) and the tile-width tuner --
+runs inside the library.  torch is used for device memory and streams only.
+
+There is no CPU fallback: importing works without a GPU (so the symbols can be checked), but every compute
+call raises `SweptError` if the library or a CUDA device is missing.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+HEAT, KS, EULER = 0, 1, 2
+F32, F64 = 0, 1
+KERNEL_SMEM, KERNEL_WAVE = 0, 1
+OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH = 0, 1, 2, 3, 4
+OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
+PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
+RADIUS = {HEAT: 1, KS: 2, EULER: 2}
+STAGES = {HEAT: 1, KS: 2, EULER: 2}
+NCOMP = {HEAT: 1, KS: 1, EULER: 3}
+
+# every symbol include/swept1d.h declares
+SYMBOLS = (
+    "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
+    "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version",
+)
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libswept1d.so")
+
+
+class SweptError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"[{code}] {message}")
+        self.code = code
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("dtype", ctypes.c_int), ("alpha", ctypes.c_double), ("gamma", ctypes.c_double), ("max_tile_width", ctypes.c_int)]
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [
+        ("problem", ctypes.c_int), ("dtype", ctypes.c_int), ("radius", ctypes.c_int), ("stages", ctypes.c_int), ("ncomp", ctypes.c_int),
+        ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
+        ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
+        ("max_smem_per_block", ctypes.c_int),
+    ]
+
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the CUDA sources in-tree (nvcc, sm_100a)."""
+    from . import _build
+    return _build.build(force=force)
+
+
+def lib() -> ctypes.CDLL:
+    """Load libswept1d.so (building it if the sources are newer).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH) or os.environ.get("SWEPT1D_REBUILD"):
+        build()
+    if not os.path.exists(LIB_PATH):
+        raise SweptError(ECUDA, f"{LIB_PATH} is missing and could not be built; there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    L.swept_create.argtypes = [ctypes.POINTER(vp), ci, i64, dbl, dbl, ctypes.POINTER(_Params)]
+    L.swept_run.argtypes = [vp, vp, i64, ci, vp]
+    L.naive_run.argtypes = [vp, vp, i64, vp]
+    L.swept_tune.argtypes = [vp, vp, ci, ctypes.POINTER(ci), vp]
+    L.swept_run_host.argtypes = [vp, vp, i64, ci, ci, vp]
+    L.swept_set_option.argtypes = [vp, ci, ci]
+    L.swept_get_info.argtypes = [vp, ctypes.POINTER(_Info)]
+    L.swept_tile_width_ok.argtypes = [vp, ci]
+    L.swept_measure_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
+    L.swept_destroy.argtypes = [vp]
+    for name in SYMBOLS:
+        getattr(L, name).restype = ci
+    L.swept_last_error.restype = ctypes.c_char_p
+    L.swept_last_error.argtypes = []
+    L.swept_version.restype = ctypes.c_char_p
+    L.swept_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise SweptError(rc, lib().swept_last_error().decode("utf-8", "replace"))
+
+
+def version() -> str:
+    return lib().swept_version().decode()
+
+
+def _stream_ptr(stream) -> int:
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream) if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dtype_id(dtype) -> int:
+    import torch
+    if dtype in (F32, F64) and not isinstance(dtype, torch.dtype):
+        return int(dtype)
+    if dtype == torch.float64:
+        return F64
+    if dtype == torch.float32:
+        return F32
+    raise SweptError(EINVAL, f"unsupported dtype {dtype}")
+
+
+class Solver:
+    """One `swept_create` handle.  `u` arguments are CUDA torch tensors of shape [ncomp, nx] (or [nx] when
+    ncomp == 1), contiguous, of the handle's dtype; they are advanced IN PLACE and asynchronously on `stream`."""
+
+    def __init__(self, problem, nx: int, dx: float, dt: float, *, dtype=F64, alpha: float = 1.0, gamma: float = 1.4,
+                 max_tile_width: int = 0):
+        if isinstance(problem, str):
+            problem = PROBLEMS[problem]
+        self._h = ctypes.c_void_p()
+        self.problem, self.nx, self.dtype = int(problem), int(nx), _dtype_id(dtype)
+        p = _Params(self.dtype, float(alpha), float(gamma), int(max_tile_width))
+        _check(lib().swept_create(ctypes.byref(self._h), self.problem, self.nx, float(dx), float(dt), ctypes.byref(p)))
+
+    # -- marshalling ----------------------------------------------------------------------------------------
+    def _ptr(self, u) -> int:
+        import torch
+        want = torch.float64 if self.dtype == F64 else torch.float32
+        if not (isinstance(u, torch.Tensor) and u.is_cuda and u.is_contiguous() and u.dtype == want):
+            raise SweptError(EINVAL, "u must be a contiguous CUDA tensor of the handle's dtype")
+        if u.numel() != NCOMP[self.problem] * self.nx:
+            raise SweptError(EINVAL, f"u must hold ncomp*nx = {NCOMP[self.problem] * self.nx} elements")
+        return u.data_ptr()
+
+    def swept_run(self, u, nsteps: int, tile_width: int = 0, stream=None) -> None:
+        _check(lib().swept_run(self._h, self._ptr(u), int(nsteps), int(tile_width), _stream_ptr(stream)))
+
+    def naive_run(self, u, nsteps: int, stream=None) -> None:
+        _check(lib().naive_run(self._h, self._ptr(u), int(nsteps), _stream_ptr(stream)))
+
+    def tune(self, scratch, blocks_per_sm_cap: int = 0, stream=None) -> int:
+        best = ctypes.c_int(0)
+        _check(lib().swept_tune(self._h, self._ptr(scratch), int(blocks_per_sm_cap), ctypes.byref(best), _stream_ptr(stream)))
+        return best.value
+
+    def run_host(self, h_u, nsteps: int, tile_width: int = 0, use_swept: bool = True, stream=None) -> None:
+        """h_u: CPU torch tensor or numpy array ([ncomp, nx], contiguous, the handle's dtype; pinned is best); updated in place."""
+        import numpy as np
+        import torch
+        if isinstance(h_u, torch.Tensor):
+            if h_u.is_cuda or not h_u.is_contiguous():
+                raise SweptError(EINVAL, "h_u must be a contiguous CPU tensor")
+            ptr, n, es = h_u.data_ptr(), h_u.numel(), h_u.element_size()
+        elif isinstance(h_u, np.ndarray) and h_u.flags["C_CONTIGUOUS"]:
+            ptr, n, es = h_u.ctypes.data, h_u.size, h_u.itemsize
+        else:
+            raise SweptError(EINVAL, "h_u must be a contiguous CPU tensor or numpy array")
+        if n != NCOMP[self.problem] * self.nx or es != (8 if self.dtype == F64 else 4):
+            raise SweptError(EINVAL, "h_u has the wrong size or dtype")
+        _check(lib().swept_run_host(self._h, ptr, int(nsteps), int(tile_width), 1 if use_swept else 0, _stream_ptr(stream)))
+
+    def set_option(self, key: int, value: int) -> None:
+        _check(lib().swept_set_option(self._h, int(key), int(value)))
+
+    def tile_width_ok(self, tile_width: int) -> bool:
+        return bool(lib().swept_tile_width_ok(self._h, int(tile_width)))
+
+    def info(self) -> dict:
+        i = _Info()
+        _check(lib().swept_get_info(self._h, ctypes.byref(i)))
+        return {name: getattr(i, name) for name, _ in _Info._fields_}
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().swept_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def measure_alu_peak(dtype=F64, stream=None) -> dict:
+    """FMA-chain microbenchmark: thread-level FP instructions per second of the FP64 / FP32 pipe."""
+    ips, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().swept_measure_alu_peak(_dtype_id(dtype), ctypes.byref(ips), ctypes.byref(ms), _stream_ptr(stream)))
+    return {"instr_per_s": ips.value, "ms": ms.value}
+
+
+def steps_per_half_cycle(problem: int, tile_width: int) -> int:
+    """L/S: full timesteps one half-cycle advances."""
+    return tile_width // (2 * RADIUS[problem] * STAGES[problem])

@@ -1,0 +1,60 @@
+// alu_peak.cu -- FMA-chain microbenchmark: the plain-ALU peak (FP64 or FP32 pipe) that bounds the swept
+// kernels ("Swept path -> plain ALUs ... never tensor cores").  Each thread runs
+// CHAINS independent fused multiply-adds per iteration, so the pipe, not latency, limits it.
+#include "internal.h"
+
+namespace swept {
+
+template <class T, int CHAINS>
+__global__ void __launch_bounds__(256) alu_peak_kernel(T *out, int iters, T a, T b) {
+    T acc[CHAINS];
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) acc[i] = (T)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < CHAINS; ++i) acc[i] = (sizeof(T) == 8) ? (T)fma((double)acc[i], (double)a, (double)b) : (T)fmaf((float)acc[i], (float)a, (float)b);
+    }
+    T sum = 0;
+#pragma unroll
+    for (int i = 0; i < CHAINS; ++i) sum += acc[i];
+    if (sum == (T)123456789) out[0] = sum;   // never true for the given a, b; keeps the chain alive
+}
+
+template <class T> static cudaError_t run_peak(int sm_count, double *instr_per_s, double *ms_out, cudaStream_t st) {
+    constexpr int CHAINS = 8;
+    T *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, sizeof(T));
+    if (e != cudaSuccess) return e;
+    const int blocks = sm_count * 8, threads = 256;
+    const int iters = sizeof(T) == 8 ? 8192 : 16384;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {   // first repetition is the warm-up
+        cudaEventRecord(e0, st);
+        alu_peak_kernel<T, CHAINS><<<blocks, threads, 0, st>>>(d, iters, (T)0.999, (T)0.001);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    if (e != cudaSuccess) return e;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const double n = (double)blocks * threads * (double)iters * CHAINS;
+    if (instr_per_s) *instr_per_s = n / (best * 1e-3);
+    if (ms_out) *ms_out = best;
+    return cudaSuccess;
+}
+
+cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st) {
+    return dtype == SWEPT_F64 ? run_peak<double>(sm_count, instr_per_s, ms, st) : run_peak<float>(sm_count, instr_per_s, ms, st);
+}
+
+}  // namespace swept

@@ -1,0 +1,465 @@
+// api.cu -- the C ABI of libswept1d.so (include/swept1d.h): handle, host driver,
+// tuner (row A8), options.  No CPU fallback: every compute entry point needs a CUDA device.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "internal.h"
+#include "stencils.cuh"
+
+using namespace swept;
+
+struct swept_ctx {
+    int problem, dtype, H, S, NC;
+    int64_t nx;
+    double dx, dt, alpha, gamma;
+    ConstBlock cb;
+    void *work;            // row R1 of the staircase / the classic path's second buffer: NC*nx elements
+    size_t field_bytes;    // NC*nx*sizeof(T)
+    void *host_stage;      // device buffer for swept_run_host (allocated on first use)
+    int device, sm_count, max_smem;
+    int kernel, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
+    int max_tile_width, tuned_tile_width;
+    int64_t launches_last, launches_total;
+    // cached CUDA graphs (one per path; rebuilt when the key changes)
+    cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
+    cudaGraphExec_t sgraph;  void *sgraph_u;  int64_t sgraph_steps;  int sgraph_W, sgraph_kernel;
+    int64_t sgraph_launches;
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...) __attribute__((format(printf, 2, 3)));
+static int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+static int fail_cuda(cudaError_t e, const char *what) {
+    cudaGetLastError();   // clear the sticky-less error state
+    return fail(SWEPT_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+extern "C" const char *swept_last_error(void) { return g_err; }
+extern "C" const char *swept_version(void) { return "swept1d-b200 0.1 (sm_100a)"; }
+
+static bool is_pow2(int64_t n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// ---- row A0: scheme constants, computed once on the host in double, then cast to the run dtype ------------
+template <class T> static void fill_consts(swept_ctx *h) {
+    memset(h->cb.bytes, 0, sizeof h->cb.bytes);
+    if (h->problem == SWEPT_HEAT) {
+        typename Heat<T>::Consts c;
+        const double Fo = h->alpha * h->dt / (h->dx * h->dx);
+        c.Fo = (T)Fo;
+        c.c0 = (T)(1.0 - 2.0 * Fo);
+        memcpy(h->cb.bytes, &c, sizeof c);
+    } else if (h->problem == SWEPT_KS) {
+        typename KS<T>::Consts c;
+        const double c2 = 1.0 / (h->dx * h->dx);                        // stored reciprocals
+        c.c1 = (T)(0.25 / h->dx);
+        c.c2 = (T)c2;
+        c.c4 = (T)(c2 * c2);
+        c.dt = (T)h->dt;
+        c.dth = (T)(0.5 * h->dt);
+        memcpy(h->cb.bytes, &c, sizeof c);
+    } else {
+        typename Euler<T>::Consts c;
+        const double lam = h->dt / h->dx;
+        c.gamma = (T)h->gamma;
+        c.gm1 = (T)(h->gamma - 1.0);
+        c.lam = (T)lam;
+        c.lamh = (T)(0.5 * lam);
+        memcpy(h->cb.bytes, &c, sizeof c);
+    }
+}
+
+extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double dx, double dt, const swept_params_t *p) {
+    g_err[0] = 0;
+    if (!out) return fail(SWEPT_EINVAL, "swept_create: out is NULL");
+    *out = nullptr;
+    if (problem != SWEPT_HEAT && problem != SWEPT_KS && problem != SWEPT_EULER) return fail(SWEPT_EINVAL, "swept_create: unknown problem %d", problem);
+    const int dtype = p ? p->dtype : SWEPT_F64;
+    if (dtype != SWEPT_F32 && dtype != SWEPT_F64) return fail(SWEPT_EINVAL, "swept_create: unknown dtype %d", dtype);
+    if (!is_pow2(nx) || nx < 8) return fail(SWEPT_EINVAL, "swept_create: nx=%lld must be a power of two >= 8 (periodic index is & (nx-1))", (long long)nx);
+    if (nx > ((int64_t)1 << 40)) return fail(SWEPT_EINVAL, "swept_create: nx too large");
+    if (!isfinite(dx) || !isfinite(dt) || dx <= 0.0 || dt <= 0.0) return fail(SWEPT_EINVAL, "swept_create: dx and dt must be finite and positive");
+    const double alpha = p ? p->alpha : 1.0, gamma = p ? p->gamma : 1.4;
+    if (problem == SWEPT_HEAT && !(isfinite(alpha) && alpha > 0.0)) return fail(SWEPT_EINVAL, "swept_create: alpha must be finite and positive");
+    if (problem == SWEPT_EULER && !(isfinite(gamma) && gamma > 1.0)) return fail(SWEPT_EINVAL, "swept_create: gamma must be finite and > 1");
+    if (p && p->max_tile_width < 0) return fail(SWEPT_EINVAL, "swept_create: max_tile_width < 0");
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_create: no CUDA device (this library has no CPU fallback)");
+    swept_ctx *h = new (std::nothrow) swept_ctx();
+    if (!h) return fail(SWEPT_ENOMEM, "swept_create: out of host memory");
+    memset(h, 0, sizeof *h);
+    h->problem = problem; h->dtype = dtype;
+    h->H = radius_of(problem); h->S = stages_of(problem); h->NC = ncomp_of(problem);
+    h->nx = nx; h->dx = dx; h->dt = dt; h->alpha = alpha; h->gamma = gamma;
+    h->device = dev;
+    h->kernel = SWEPT_KERNEL_WAVE;
+    h->warps_per_block = 4;
+    h->max_tile_width = p ? p->max_tile_width : 0;
+    if (dtype == SWEPT_F64) fill_consts<double>(h); else fill_consts<float>(h);
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&h->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    h->field_bytes = (size_t)h->NC * (size_t)nx * elem_size(dtype);
+    e = cudaMalloc(&h->work, h->field_bytes);
+    if (e != cudaSuccess) {
+        delete h;
+        cudaGetLastError();
+        return fail(e == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "swept_create: cudaMalloc workspace: %s", cudaGetErrorString(e));
+    }
+    e = swept_smem_prepare(problem, dtype, (size_t)h->max_smem);
+    if (e == cudaSuccess) e = swept_wave_prepare(problem, dtype);
+    if (e != cudaSuccess) { cudaFree(h->work); delete h; return fail_cuda(e, "swept_create: kernel attribute setup"); }
+    *out = h;
+    return SWEPT_OK;
+}
+
+static void drop_graphs(swept_ctx *h) {
+    if (h->ngraph) { cudaGraphExecDestroy(h->ngraph); h->ngraph = nullptr; }
+    if (h->sgraph) { cudaGraphExecDestroy(h->sgraph); h->sgraph = nullptr; }
+}
+
+extern "C" int swept_destroy(swept_handle_t h) {
+    if (!h) return fail(SWEPT_EINVAL, "swept_destroy: NULL handle");
+    drop_graphs(h);
+    if (h->work) cudaFree(h->work);
+    if (h->host_stage) cudaFree(h->host_stage);
+    delete h;
+    return SWEPT_OK;
+}
+
+// ---- legality of a tile width (SURVEY.md section 8(a) "Legal tile widths") ------------------------------------
+static int check_width(const swept_ctx *h, int W, int kernel, bool set_err) {
+    const char *why = nullptr;
+    char buf[160];
+    if (W <= 0 || !is_pow2(W)) why = "tile width must be a power of two";
+    else if (W < 4 * h->H) why = "tile width must be >= 4h (L = W/(2h) even)";
+    else if ((int64_t)W > h->nx) why = "tile width exceeds nx";
+    else if (kernel == SWEPT_KERNEL_SMEM) {
+        const size_t need = swept_smem_bytes(h->problem, h->dtype, W);
+        if (need > (size_t)h->max_smem) {
+            snprintf(buf, sizeof buf, "tile needs %zu B of shared memory, limit %d B", need, h->max_smem);
+            why = buf;
+        }
+    } else if (kernel == SWEPT_KERNEL_WAVE) {
+        if (!swept_wave_supports(h->problem, h->dtype, W)) why = "tile width not supported by the WAVE kernels for this problem/dtype";
+    } else why = "unknown kernel";
+    if (why) {
+        if (set_err) fail(SWEPT_EINVAL, "tile_width %d: %s", W, why);
+        return 0;
+    }
+    return 1;
+}
+
+extern "C" int swept_tile_width_ok(swept_handle_t h, int tile_width) {
+    if (!h) { fail(SWEPT_EINVAL, "swept_tile_width_ok: NULL handle"); return 0; }
+    return check_width(h, tile_width, h->kernel, true);
+}
+
+static int default_width(const swept_ctx *h) {
+    if (h->tuned_tile_width) return h->tuned_tile_width;
+    // largest legal width not above 256 (WAVE) / 512 (SMEM) and nx
+    for (int W = h->kernel == SWEPT_KERNEL_WAVE ? 256 : 512; W >= 4 * h->H; W >>= 1)
+        if (check_width(h, W, h->kernel, false)) return W;
+    return 0;
+}
+
+// ---- classic path (row A2) -----------------------------------------------------------------------------------
+// Enqueue nsteps classic timesteps.  Heat ping-pongs u and work (and copies back after an odd count); two-stage
+// schemes write the predictor to work and accumulate the final stage onto u (Fig. 6).
+static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cudaStream_t st, int64_t *launches) {
+    cudaError_t e = cudaSuccess;
+    if (h->S == 1) {
+        void *a = d_u, *b = h->work;
+        for (int64_t m = 0; m < nsteps; ++m) {
+            e = launch_classic_stage(h->problem, h->dtype, 1, a, a, b, h->nx, h->cb, st);
+            if (e != cudaSuccess) return e;
+            void *t = a; a = b; b = t;
+            ++*launches;
+        }
+        if (a != d_u) {
+            e = cudaMemcpyAsync(d_u, a, h->field_bytes, cudaMemcpyDeviceToDevice, st);
+            ++*launches;
+        }
+    } else {
+        for (int64_t m = 0; m < nsteps; ++m) {
+            e = launch_classic_stage(h->problem, h->dtype, 1, d_u, d_u, h->work, h->nx, h->cb, st);
+            if (e != cudaSuccess) return e;
+            e = launch_classic_stage(h->problem, h->dtype, 0, h->work, d_u, d_u, h->nx, h->cb, st);
+            if (e != cudaSuccess) return e;
+            *launches += 2;
+        }
+    }
+    return e;
+}
+
+static int run_args_ok(swept_ctx *h, void *d_u, int64_t nsteps, const char *who) {
+    if (!h) return fail(SWEPT_EINVAL, "%s: NULL handle", who);
+    if (!d_u) return fail(SWEPT_EINVAL, "%s: d_u is NULL", who);
+    if (nsteps < 0) return fail(SWEPT_EINVAL, "%s: nsteps < 0", who);
+    if (((uintptr_t)d_u & 15) != 0) return fail(SWEPT_EINVAL, "%s: d_u must be 16-byte aligned", who);
+    return SWEPT_OK;
+}
+
+// Replay `steps` of a path through a cached CUDA graph (captured on first use with the same key).
+template <class Enqueue>
+static int run_graphed(cudaGraphExec_t *exec, bool reuse, cudaStream_t st, int64_t *launches, Enqueue &&enq, const char *who) {
+    cudaError_t e;
+    if (!reuse) {
+        if (*exec) { cudaGraphExecDestroy(*exec); *exec = nullptr; }
+        cudaStream_t cap;
+        e = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return fail_cuda(e, who);
+        e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+        if (e != cudaSuccess) { cudaStreamDestroy(cap); return fail_cuda(e, who); }
+        *launches = 0;
+        cudaError_t el = enq(cap, launches);
+        cudaGraph_t g = nullptr;
+        e = cudaStreamEndCapture(cap, &g);
+        cudaStreamDestroy(cap);
+        if (el != cudaSuccess) { if (g) cudaGraphDestroy(g); return fail_cuda(el, who); }
+        if (e != cudaSuccess) return fail_cuda(e, who);
+        e = cudaGraphInstantiate(exec, g, 0);
+        cudaGraphDestroy(g);
+        if (e != cudaSuccess) { *exec = nullptr; return fail_cuda(e, who); }
+    }
+    e = cudaGraphLaunch(*exec, st);
+    if (e != cudaSuccess) return fail_cuda(e, who);
+    return SWEPT_OK;
+}
+
+extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream) {
+    int rc = run_args_ok(h, d_u, nsteps, "naive_run");
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int64_t launches = 0;
+    if (h->naive_graph && nsteps >= 2) {
+        // a graph of `chunk` timesteps (even, so heat's ping-pong ends in d_u), replayed; the rest as plain launches
+        int64_t chunk = nsteps < 1000 ? nsteps : 1000;
+        chunk -= chunk & 1;
+        const bool reuse = h->ngraph && h->ngraph_u == d_u && h->ngraph_steps == chunk;
+        const int64_t reps = nsteps / chunk;
+        for (int64_t i = 0; i < reps; ++i) {
+            int64_t l = 0;
+            rc = run_graphed(&h->ngraph, reuse || i > 0, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_classic(h, d_u, chunk, s, n); }, "naive_run(graph)");
+            if (rc) return rc;
+            if (!reuse && i == 0) { h->ngraph_u = d_u; h->ngraph_steps = chunk; h->ngraph_launches = l; }
+            launches += h->ngraph_launches;
+        }
+        cudaError_t e = enqueue_classic(h, d_u, nsteps % chunk, st, &launches);
+        if (e != cudaSuccess) return fail_cuda(e, "naive_run");
+    } else {
+        cudaError_t e = enqueue_classic(h, d_u, nsteps, st, &launches);
+        if (e != cudaSuccess) return fail_cuda(e, "naive_run");
+    }
+    h->launches_last = launches;
+    h->launches_total += launches;
+    return SWEPT_OK;
+}
+
+// ---- swept path (row A7) ---------------------------------------------------------------------------------------
+static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, int W, int64_t offset, cudaStream_t st) {
+    if (kernel == SWEPT_KERNEL_SMEM) return launch_swept_smem(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, st);
+    return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, h->blocks_per_sm, st);
+}
+
+// q half-cycles of width W: 1 upright triangle + (q-1) diamonds on tiles shifted by W/2 each launch + 1 closing
+// inverted triangle.  On a periodic domain either alignment may write out (reading S4).
+static cudaError_t enqueue_half_cycles(swept_ctx *h, int kernel, void *d_u, int W, int64_t q, cudaStream_t st, int64_t *launches) {
+    if (q <= 0) return cudaSuccess;
+    cudaError_t e = launch_phase(h, kernel, MODE_UP, d_u, W, 0, st);
+    if (e != cudaSuccess) return e;
+    for (int64_t i = 1; i < q; ++i) {
+        e = launch_phase(h, kernel, MODE_DIAMOND, d_u, W, (i & 1) ? W / 2 : 0, st);
+        if (e != cudaSuccess) return e;
+    }
+    e = launch_phase(h, kernel, MODE_DOWN, d_u, W, (q & 1) ? W / 2 : 0, st);
+    *launches += q + 1;
+    return e;
+}
+
+// nsteps = q*(L/S) + r.  The r remaining timesteps run first (reading S3): on successively narrower legal tiles
+// (each one half-cycle: one upright + one closing triangle), and what no tile width divides on the classic kernel.
+static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches) {
+    const int per = 2 * h->H * h->S;   // W / per = timesteps per half-cycle
+    const int64_t sph = W / per;
+    const int64_t q = nsteps / sph;
+    int64_t r = nsteps % sph;
+    cudaError_t e = cudaSuccess;
+    for (int w = W / 2; w >= 4 * h->H && r > 0; w >>= 1) {
+        const int64_t s = w / per;
+        if (s >= 1 && r >= s && check_width(h, w, kernel, false)) {
+            e = enqueue_half_cycles(h, kernel, d_u, w, 1, st, launches);
+            if (e != cudaSuccess) return e;
+            r -= s;
+        }
+    }
+    if (r > 0) {
+        e = enqueue_classic(h, d_u, r, st, launches);
+        if (e != cudaSuccess) return e;
+    }
+    return enqueue_half_cycles(h, kernel, d_u, W, q, st, launches);
+}
+
+extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void *cuda_stream) {
+    int rc = run_args_ok(h, d_u, nsteps, "swept_run");
+    if (rc) return rc;
+    int W = tile_width;
+    if (W == 0) {
+        W = default_width(h);
+        if (W == 0) return fail(SWEPT_EINVAL, "swept_run: no legal tile width for nx=%lld with the selected kernel", (long long)h->nx);
+    } else if (!check_width(h, W, h->kernel, true)) return SWEPT_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int64_t launches = 0;
+    if (h->swept_graph && nsteps > 0) {
+        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel;
+        int64_t l = 0;
+        rc = run_graphed(&h->sgraph, reuse, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_swept(h, h->kernel, d_u, nsteps, W, s, n); }, "swept_run(graph)");
+        if (rc) return rc;
+        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_launches = l; }
+        launches = h->sgraph_launches;
+    } else {
+        cudaError_t e = enqueue_swept(h, h->kernel, d_u, nsteps, W, st, &launches);
+        if (e != cudaSuccess) return fail_cuda(e, "swept_run");
+    }
+    h->launches_last = launches;
+    h->launches_total += launches;
+    return SWEPT_OK;
+}
+
+// ---- tuner (row A8; "best node size") -----------------------------------------------------------
+extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream) {
+    int rc = run_args_ok(h, d_u_scratch, 0, "swept_tune");
+    if (rc) return rc;
+    if (blocks_per_sm_cap < 0) return fail(SWEPT_EINVAL, "swept_tune: blocks_per_sm_cap < 0");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int saved_cap = h->blocks_per_sm, saved_graph = h->swept_graph;
+    h->blocks_per_sm = blocks_per_sm_cap;
+    h->swept_graph = 0;
+    int wmax = h->max_tile_width ? h->max_tile_width : 4096;
+    if ((int64_t)wmax > h->nx) wmax = (int)h->nx;
+    int wtop = 0;
+    for (int W = 4 * h->H; W <= wmax; W <<= 1) if (check_width(h, W, h->kernel, false)) wtop = W;
+    if (!wtop) { h->blocks_per_sm = saved_cap; h->swept_graph = saved_graph; return fail(SWEPT_EINVAL, "swept_tune: no legal tile width"); }
+    // every candidate advances the same number of timesteps: four half-cycles of the widest tile
+    const int64_t nsteps = 4 * (int64_t)(wtop / (2 * h->H * h->S));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    int best = 0;
+    float best_ms = 1e30f;
+    cudaError_t e = cudaSuccess;
+    for (int W = 4 * h->H; W <= wtop && e == cudaSuccess; W <<= 1) {
+        if (!check_width(h, W, h->kernel, false)) continue;
+        float ms_min = 1e30f;
+        for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
+            int64_t l = 0;
+            cudaEventRecord(e0, st);
+            e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
+            cudaEventRecord(e1, st);
+            if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+            float ms = 0;
+            if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < ms_min) ms_min = ms;
+            h->launches_total += l;
+        }
+        if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    h->blocks_per_sm = saved_cap;
+    h->swept_graph = saved_graph;
+    if (e != cudaSuccess) return fail_cuda(e, "swept_tune");
+    h->tuned_tile_width = best;
+    if (best_tile_width) *best_tile_width = best;
+    return SWEPT_OK;
+}
+
+// ---- end-to-end convenience: host buffer in, host buffer out -------------------------------------------------
+extern "C" int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int tile_width, int use_swept, void *cuda_stream) {
+    if (!h) return fail(SWEPT_EINVAL, "swept_run_host: NULL handle");
+    if (!h_u) return fail(SWEPT_EINVAL, "swept_run_host: h_u is NULL");
+    if (nsteps < 0) return fail(SWEPT_EINVAL, "swept_run_host: nsteps < 0");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (!h->host_stage) {
+        e = cudaMalloc(&h->host_stage, h->field_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); h->host_stage = nullptr; return fail(SWEPT_ENOMEM, "swept_run_host: cudaMalloc: %s", cudaGetErrorString(e)); }
+    }
+    e = cudaMemcpyAsync(h->host_stage, h_u, h->field_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_run_host: H2D");
+    int rc = use_swept ? swept_run(h, h->host_stage, nsteps, tile_width, cuda_stream) : naive_run(h, h->host_stage, nsteps, cuda_stream);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(h_u, h->host_stage, h->field_bytes, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_run_host: D2H");
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_run_host: synchronize");
+    return SWEPT_OK;
+}
+
+extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
+    if (!h) return fail(SWEPT_EINVAL, "swept_set_option: NULL handle");
+    switch (key) {
+        case SWEPT_OPT_KERNEL:
+            if (value != SWEPT_KERNEL_SMEM && value != SWEPT_KERNEL_WAVE) return fail(SWEPT_EINVAL, "swept_set_option: unknown kernel %d", value);
+            if (value != h->kernel) h->tuned_tile_width = 0;
+            h->kernel = value;
+            return SWEPT_OK;
+        case SWEPT_OPT_NAIVE_GRAPH:
+            if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: NAIVE_GRAPH takes 0 or 1");
+            h->naive_graph = value;
+            return SWEPT_OK;
+        case SWEPT_OPT_SWEPT_GRAPH:
+            if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: SWEPT_GRAPH takes 0 or 1");
+            h->swept_graph = value;
+            return SWEPT_OK;
+        case SWEPT_OPT_BLOCKS_PER_SM:
+            if (value < 0 || value > 32) return fail(SWEPT_EINVAL, "swept_set_option: BLOCKS_PER_SM takes 0..32");
+            h->blocks_per_sm = value;
+            drop_graphs(h);
+            return SWEPT_OK;
+        case SWEPT_OPT_WARPS_PER_BLOCK:
+            if (value != 1 && value != 2 && value != 4 && value != 8 && value != 16) return fail(SWEPT_EINVAL, "swept_set_option: WARPS_PER_BLOCK takes 1, 2, 4, 8 or 16");
+            h->warps_per_block = value;
+            drop_graphs(h);
+            return SWEPT_OK;
+        default:
+            return fail(SWEPT_EINVAL, "swept_set_option: unknown key %d", key);
+    }
+}
+
+extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
+    if (!h || !info) return fail(SWEPT_EINVAL, "swept_get_info: NULL argument");
+    info->problem = h->problem; info->dtype = h->dtype;
+    info->radius = h->H; info->stages = h->S; info->ncomp = h->NC;
+    info->nx = h->nx;
+    info->workspace_bytes = (int64_t)h->field_bytes;
+    info->tuned_tile_width = h->tuned_tile_width;
+    info->launches_last_call = h->launches_last;
+    info->launches_total = h->launches_total;
+    info->sm_count = h->sm_count;
+    info->max_smem_per_block = h->max_smem;
+    return SWEPT_OK;
+}
+
+extern "C" int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms, void *cuda_stream) {
+    if (dtype != SWEPT_F32 && dtype != SWEPT_F64) return fail(SWEPT_EINVAL, "swept_measure_alu_peak: unknown dtype %d", dtype);
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_measure_alu_peak: no CUDA device");
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    e = run_alu_peak(dtype, sms, instr_per_s, ms, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_measure_alu_peak");
+    return SWEPT_OK;
+}

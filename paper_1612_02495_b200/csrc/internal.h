@@ -1,0 +1,59 @@
+// internal.h -- declarations shared by the translation units of libswept1d.so (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/swept1d.h"
+
+namespace swept {
+
+// Scheme constants of one handle, stored as the bytes of P<T>::Consts (row A0; the paper keeps them in a
+// __constant__ struct, PAPER.md:42, 193 -- here they travel as a by-value kernel parameter, which lives in
+// the same constant bank).
+struct ConstBlock {
+    alignas(8) unsigned char bytes[64];
+};
+
+enum { MODE_UP = 0, MODE_DIAMOND = 1, MODE_DOWN = 2 };
+
+// One classic sub-timestep over all nx points (naive.cu).  odd: predictor stage of a two-stage scheme.
+// dst[i] = stage(win_src[i-H..i+H], base[i]); base may alias dst.
+cudaError_t launch_classic_stage(int problem, int dtype, int odd, const void *win_src, const void *base, void *dst,
+                                 int64_t nx, const ConstBlock &cb, cudaStream_t st);
+
+// Paper-style shared-memory swept kernels (swept_smem.cu): one block per tile of W points.
+// mode: MODE_UP | MODE_DIAMOND | MODE_DOWN; offset: tile-grid shift (0 or W/2).
+cudaError_t launch_swept_smem(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
+                              const ConstBlock &cb, cudaStream_t st);
+size_t swept_smem_bytes(int problem, int dtype, int W);
+cudaError_t swept_smem_prepare(int problem, int dtype, size_t max_bytes);
+
+// Register-resident wavefront swept kernels (swept_wave.cu): one warp per tile of W points.
+cudaError_t launch_swept_wave(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
+                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, cudaStream_t st);
+int swept_wave_supports(int problem, int dtype, int W);
+cudaError_t swept_wave_prepare(int problem, int dtype);
+
+// FMA-chain microbenchmark (alu_peak.cu)
+cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st);
+
+inline int radius_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }
+inline int stages_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }
+inline int ncomp_of(int problem) { return problem == SWEPT_EULER ? 3 : 1; }
+inline size_t elem_size(int dtype) { return dtype == SWEPT_F64 ? 8 : 4; }
+
+}  // namespace swept
+
+// Dispatch a (problem, dtype) pair to a template taking <P<T>>: SWEPT_DISPATCH(problem, dtype, P, expr-using-P)
+#define SWEPT_DISPATCH(problem, dtype, PNAME, ...)                                                        \
+    do {                                                                                                  \
+        if ((dtype) == SWEPT_F64) {                                                                       \
+            if ((problem) == SWEPT_HEAT) { using PNAME = ::swept::Heat<double>; __VA_ARGS__; }            \
+            else if ((problem) == SWEPT_KS) { using PNAME = ::swept::KS<double>; __VA_ARGS__; }           \
+            else { using PNAME = ::swept::Euler<double>; __VA_ARGS__; }                                   \
+        } else {                                                                                          \
+            if ((problem) == SWEPT_HEAT) { using PNAME = ::swept::Heat<float>; __VA_ARGS__; }             \
+            else if ((problem) == SWEPT_KS) { using PNAME = ::swept::KS<float>; __VA_ARGS__; }            \
+            else { using PNAME = ::swept::Euler<float>; __VA_ARGS__; }                                    \
+        }                                                                                                 \
+    } while (0)

@@ -1,0 +1,224 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, and the swept
+kernels against the classic kernel bit for bit (include/swept1d.h guarantee; north_star).
+
+Tolerance (north_star): relative max-norm <= 1e-12 (fp64) / 1e-5 (fp32) against the oracle.  Oracle and CUDA path
+evaluate the same canonical operation order with explicit fma and no contraction, so the
+tests additionally assert the stronger statement that holds by construction: identical bits.
+"""
+import numpy as np
+import pytest
+
+import paper_1612_02495_b200 as sw
+import workloads as wl
+from gpu_util import (TOL, assert_bits_equal, rel_max, run_naive, run_oracle, run_swept, solver_for, to_dev, width_ok)
+
+pytestmark = pytest.mark.gpu
+
+PROBLEMS = [wl.HEAT, wl.KS, wl.EULER]
+DTYPES = [np.float64, np.float32]
+KERNELS = [sw.KERNEL_SMEM, sw.KERNEL_WAVE]
+KNAME = {sw.KERNEL_SMEM: "smem", sw.KERNEL_WAVE: "wave"}
+
+
+def _noise(problem, nx):
+    return wl.make(problem, nx, "noise")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# classic (naive) path vs oracle
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+@pytest.mark.parametrize("nx,nsteps", [(8, 3), (64, 37), (4096, 101), (1 << 16, 12)])
+def test_naive_matches_oracle(problem, dtype, nx, nsteps):
+    w = _noise(problem, nx)
+    got = run_naive(w, dtype, nsteps)
+    ref = run_oracle(w, dtype, nsteps)
+    assert np.all(np.isfinite(ref))
+    assert rel_max(got, ref) <= TOL[dtype]
+    assert_bits_equal(got, ref, f"naive vs oracle {wl.PROBLEM_NAMES[problem]} nx={nx}")
+
+
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+def test_naive_zero_steps_is_identity_and_graph_matches_plain(problem):
+    w = _noise(problem, 1024)
+    u0 = w.initial(np.float64)
+    assert_bits_equal(run_naive(w, np.float64, 0), u0, "0 steps")
+    assert_bits_equal(run_naive(w, np.float64, 57, graph=True), run_naive(w, np.float64, 57), "graph vs plain")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# swept vs classic: bit-exact for every legal tile width, remainder, alignment, single-tile wrap
+# ------------------------------------------------------------------------------------------------------------
+def _sph(problem, W):
+    return wl.steps_per_half_cycle(problem, W)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+@pytest.mark.parametrize("W", [8, 32, 64, 128, 256, 512, 1024, 2048])
+def test_swept_matches_naive_bitwise(problem, dtype, W, kernel):
+    nx = max(4 * W, 2048)
+    w = _noise(problem, nx)
+    if not width_ok(w, dtype, W, kernel):
+        pytest.skip(f"W={W} not offered by the {KNAME[kernel]} kernel for this problem")
+    sph = _sph(problem, W)
+    # 3 half-cycles (odd: closes on the shifted alignment) plus a remainder that needs narrower tiles and a classic step
+    nsteps = 3 * sph + (sph // 2 + 1 if sph > 1 else 0)
+    got = run_swept(w, dtype, nsteps, W, kernel)
+    ref = run_naive(w, dtype, nsteps)
+    assert np.all(np.isfinite(ref))
+    assert_bits_equal(got, ref, f"swept({KNAME[kernel]}) vs naive W={W}")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+@pytest.mark.parametrize("q", [1, 2, 4, 5])
+def test_swept_half_cycle_counts(problem, q, kernel):
+    """Odd and even half-cycle counts both write out correctly (reading S4), q = 1 is up + down only."""
+    W, nx = 64, 1024
+    w = _noise(problem, nx)
+    if not width_ok(w, np.float64, W, kernel):
+        pytest.skip("width not offered")
+    nsteps = q * _sph(problem, W)
+    assert_bits_equal(run_swept(w, np.float64, nsteps, W, kernel), run_naive(w, np.float64, nsteps), f"q={q}")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+def test_swept_single_tile_wraps_onto_itself(problem, kernel):
+    W = nx = 256
+    w = _noise(problem, nx)
+    if not width_ok(w, np.float64, W, kernel):
+        pytest.skip("width not offered")
+    nsteps = 3 * _sph(problem, W) + 1
+    assert_bits_equal(run_swept(w, np.float64, nsteps, W, kernel), run_naive(w, np.float64, nsteps), "nx == W")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+def test_swept_translation_equivariance_bitwise(problem, kernel):
+    """A circular shift by a non-multiple of W commutes with the swept run bit for bit (exposes tile-edge bugs)."""
+    W, nx, shift = 128, 2048, 37
+    w = _noise(problem, nx)
+    if not width_ok(w, np.float64, W, kernel):
+        pytest.skip("width not offered")
+    nsteps = 2 * _sph(problem, W) + 3
+    u0 = w.initial(np.float64)
+    a = run_swept(w, np.float64, nsteps, W, kernel, u0=u0)
+    b = run_swept(w, np.float64, nsteps, W, kernel, u0=np.ascontiguousarray(np.roll(u0, shift, axis=1)))
+    assert_bits_equal(b.reshape(u0.shape), np.roll(a.reshape(u0.shape), shift, axis=1), "shift equivariance")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+def test_result_independent_of_tile_width(kernel):
+    w = _noise(wl.KS, 4096)
+    outs = []
+    for W in (32, 64, 256, 1024):
+        if width_ok(w, np.float64, W, kernel):
+            outs.append(run_swept(w, np.float64, 300, W, kernel))
+    if len(outs) < 2:
+        pytest.skip("fewer than two widths offered")
+    for o in outs[1:]:
+        assert_bits_equal(o, outs[0], "tile-width independence")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+def test_swept_graph_replay_matches_plain(kernel):
+    w = _noise(wl.HEAT, 4096)
+    if not width_ok(w, np.float64, 128, kernel):
+        pytest.skip("width not offered")
+    a = run_swept(w, np.float64, 500, 128, kernel, graph=True)
+    assert_bits_equal(a, run_naive(w, np.float64, 500), "graph replay")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# swept vs oracle on the configs (BASELINE.json)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+def test_config1_heat_full_run_matches_oracle(kernel):
+    """Config 1 exactly: heat fp64, nx=1024, r=0.25, 10 000 steps, W=64 (312 half-cycles + 16 remainder steps)."""
+    w = wl.heat_config1()
+    if not width_ok(w, np.float64, w.tile_width, kernel):
+        pytest.skip("width not offered")
+    got = run_swept(w, np.float64, w.nsteps, w.tile_width, kernel)
+    ref = run_oracle(w, np.float64, w.nsteps)
+    assert rel_max(got, ref) <= 1e-12
+    assert_bits_equal(got, ref, "config 1")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
+@pytest.mark.parametrize("problem,nx,nsteps,W", [(wl.HEAT, 1 << 14, 3000, 256), (wl.KS, 1 << 14, 2000, 256), (wl.EULER, 1 << 12, 1500, 128)],
+                         ids=["heat-c2", "ks-c3", "euler-c4"])
+def test_config_workloads_match_oracle(problem, nx, nsteps, W, dtype, kernel):
+    """Configs 2-4 initial data at their smallest nx on a prefix of the run the oracle finishes in seconds."""
+    w = wl.make(problem, nx, "config")
+    if not width_ok(w, dtype, W, kernel):
+        pytest.skip("width not offered")
+    got = run_swept(w, dtype, nsteps, W, kernel)
+    ref = run_oracle(w, dtype, nsteps)
+    assert np.all(np.isfinite(ref))
+    assert rel_max(got, ref) <= TOL[dtype]
+    assert_bits_equal(got, ref, "config workload")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# boundary behaviour
+# ------------------------------------------------------------------------------------------------------------
+def test_illegal_arguments_are_rejected():
+    import torch
+    w = _noise(wl.KS, 1024)
+    with solver_for(w, np.float64) as s:
+        s.set_option(sw.OPT_KERNEL, sw.KERNEL_SMEM)
+        u = to_dev(w.initial(np.float64))
+        for bad in (3, 4, 48, 2048, -8):
+            with pytest.raises(sw.SweptError) as ei:
+                s.swept_run(u, 10, bad)
+            assert ei.value.code == sw.EINVAL
+        with pytest.raises(sw.SweptError):
+            s.swept_run(u, -1, 64)
+        with pytest.raises(sw.SweptError):
+            s.naive_run(u.float(), 1)
+        with pytest.raises(sw.SweptError):
+            s.set_option(99, 0)
+        torch.cuda.synchronize()
+        assert_bits_equal(u.cpu().numpy(), w.initial(np.float64), "rejected calls must not touch the field")
+
+
+def test_run_host_round_trip_and_info():
+    import torch
+    w = _noise(wl.EULER, 2048)
+    with solver_for(w, np.float64) as s:
+        s.set_option(sw.OPT_KERNEL, sw.KERNEL_SMEM)
+        h = torch.from_numpy(w.initial(np.float64)).pin_memory()
+        s.run_host(h, 40, 64, use_swept=True)
+        info = s.info()
+        assert info["ncomp"] == 3 and info["radius"] == 2 and info["stages"] == 2 and info["nx"] == 2048
+        assert info["launches_last_call"] == 40 // 8 + 1
+        assert_bits_equal(h.numpy(), run_naive(w, np.float64, 40), "run_host")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+def test_tuner_returns_a_legal_width_and_default_run_uses_it(kernel):
+    import torch
+    w = _noise(wl.HEAT, 1 << 14)
+    with solver_for(w, np.float32, max_tile_width=512) as s:
+        s.set_option(sw.OPT_KERNEL, kernel)
+        if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512)):
+            pytest.skip("kernel offers no width")
+        scratch = to_dev(w.initial(np.float32))
+        best = s.tune(scratch)
+        assert s.tile_width_ok(best) and best <= 512
+        assert s.info()["tuned_tile_width"] == best
+        u = to_dev(w.initial(np.float32))
+        s.swept_run(u, 777, 0)
+        torch.cuda.synchronize()
+        assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float32, 777), "tuned width run")
+
+
+def test_alu_peak_microbenchmark_is_plausible():
+    p64 = sw.measure_alu_peak(sw.F64)["instr_per_s"]
+    p32 = sw.measure_alu_peak(sw.F32)["instr_per_s"]
+    assert 1e12 < p64 < 1e14 and 1e12 < p32 < 2e14
