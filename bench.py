@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point updates per second of the swept hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one `swept_run` call that advances
+the config-2 heat workload (FTCS, periodic, r = 0.25, 4 seeded sine modes; nx = 2^22, the largest nx of the sweep)
+by `--nsteps` timesteps (default: the config's 50 000) -- remainder kernels, upright triangle, all diamonds and the
+closing inverted triangle included.  value = nx * nsteps * K / (sum of the K CUDA-event step times).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--problem heat|ks|euler] [--dtype f64|f32] [--nx NX] [--nsteps NS] [--tile-width W] [--kernel wave|smem]
+                    [--sweep]      (also time swept vs classic over nx = 2^11..2^22, written to gpurun_out/sweep_*.json)
+
+N > 1 (torchrun, one rank per GPU): the path does not shard (north_star: one GPU, no collectives) -- every rank runs an
+independent replica ("replicas only", scaling "weak"); value = units all ranks processed / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP instructions of one point update
+    ("heat", "f64"): 3, ("heat", "f32"): 3, ("ks", "f64"): 11, ("ks", "f32"): 11, ("euler", "f64"): 0, ("euler", "f32"): 0,
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--problem", default="heat", choices=["heat", "ks", "euler"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--nx", type=int, default=1 << 22)
+    ap.add_argument("--nsteps", type=int, default=0, help="timesteps per bench step (0 = the config's count)")
+    ap.add_argument("--tile-width", type=int, default=0, help="0 = tuned (swept_tune)")
+    ap.add_argument("--kernel", default="wave", choices=["wave", "smem"])
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
+    return ap.parse_args()
+
+
+def workload(args) -> wl.Workload:
+    w = wl.make(args.problem, args.nx, "config")
+    if args.nsteps:
+        w.nsteps = args.nsteps
+    return w
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# clocks: sample nvidia-smi during the timed region (B200_PROFILING.md "clocks line")
+# ---------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# CPU baseline / reference arm: the oracle as it stands, on the host cores, bounded sample
+# ---------------------------------------------------------------------------------------------------------------
+def oracle_rate(w: wl.Workload, dtype, budget_s: float = 12.0):
+    import oracle
+    u0 = w.initial(dtype)
+    t0 = time.perf_counter()
+    oracle.run(w.problem, u0, 4, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    t4 = time.perf_counter() - t0
+    n = int(max(8, min(w.nsteps, budget_s / max(t4 / 4, 1e-9))))
+    t0 = time.perf_counter()
+    oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    dt = time.perf_counter() - t0
+    return w.nx * n / dt, n, dt, oracle.num_threads()
+
+
+def run_reference(args):
+    """--impl reference: this tier has no reference implementation; the reference arm is the CPU oracle."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = workload(args)
+    dtype = np.float64 if args.dtype == "f64" else np.float32
+    import oracle
+    u0 = w.initial(dtype)
+    t0 = time.perf_counter()
+    oracle.run(w.problem, u0, 2, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    per = (time.perf_counter() - t0) / 2
+    total = max(1, args.steps + args.warmup)
+    n = int(max(2, min(w.nsteps, (90.0 / total) / max(per, 1e-9))))    # whole run <= ~1.5 min
+    for _ in range(args.warmup):
+        oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    el = time.perf_counter() - t0
+    val = w.nx * n * args.steps / el / 1e9
+    sample = f"{n} of the config's {w.nsteps} timesteps per step at nx={w.nx} (rate is step-count independent)"
+    print(json.dumps({
+        "impl": "reference", "metric": "grid-point updates/sec", "value": val, "unit": "GPts*steps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"{w.name} nx={w.nx} {args.dtype}; CPU oracle (plain C, OpenMP) on host cores", "nx": w.nx,
+                   "nsteps_per_step": n},
+        "cpu_baseline": {"value": val, "unit": "GPts*steps/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GPts*steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_1612_02495_b200 as sw
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the swept path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    w = workload(args)
+    np_dtype = np.float64 if args.dtype == "f64" else np.float32
+    sw_dtype = sw.F64 if args.dtype == "f64" else sw.F32
+    kernel = sw.KERNEL_WAVE if args.kernel == "wave" else sw.KERNEL_SMEM
+    s = sw.Solver(w.problem, w.nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma)
+    s.set_option(sw.OPT_KERNEL, kernel)
+    if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512, 1024)):
+        kernel = sw.KERNEL_SMEM
+        s.set_option(sw.OPT_KERNEL, kernel)
+    u0_host = torch.from_numpy(w.initial(np_dtype)).pin_memory()
+    u = u0_host.cuda()
+    stream = torch.cuda.current_stream()
+    W = args.tile_width or s.tune(u.clone())
+    sph = sw.steps_per_half_cycle(w.problem, W)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, k):
+        """k calls of fn, each bracketed by CUDA events on the launching stream, L2 flushed between calls."""
+        tot = 0.0
+        for _ in range(k):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            e1.synchronize()
+            tot += e0.elapsed_time(e1) * 1e-3
+        return tot
+
+    # ---- device-resident timing: inputs already in HBM ----------------------------------------------------
+    def step_dev():
+        s.swept_run(u, w.nsteps, W)
+
+    for _ in range(max(args.warmup, 3)):
+        u.copy_(u0_host, non_blocking=True)
+        step_dev()
+    barrier()
+    l0 = s.info()["launches_total"]
+    with ClockSampler(local_rank) as clk:
+        barrier()
+        t_dev = timed(step_dev, args.steps)
+        barrier()
+    launches = s.info()["launches_total"] - l0
+    t = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    t_dev_max = float(t.item())
+    value = world * w.nx * w.nsteps * args.steps / t_dev_max / 1e9
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----------------
+    h_buf = u0_host.clone().pin_memory()
+
+    def step_e2e():
+        s.run_host(h_buf, w.nsteps, W, use_swept=True)
+
+    step_e2e()
+    barrier()
+    t_e2e = timed(step_e2e, args.steps)
+    t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = world * w.nx * w.nsteps * args.steps / float(t.item()) / 1e9
+    field_bytes = int(u.numel() * u.element_size())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the diamond): average launch duration by differencing two runs ----
+    def half_cycles(q):
+        return lambda: s.swept_run(u, q * sph, W)
+
+    qa, qb = 16, 48
+    for q in (qa, qb):
+        half_cycles(q)()
+    ta = min(timed(half_cycles(qa), 1) for _ in range(3))
+    tb = min(timed(half_cycles(qb), 1) for _ in range(3))
+    t_diamond = (tb - ta) / (qb - qa)
+    H, S = sw.RADIUS[w.problem], sw.STAGES[w.problem]
+    L = W // (2 * H)
+    stage_updates = w.nx * L                                   # per diamond launch: every point advances L tiers
+    fpi = FP_INSTR_PER_STAGE_UPDATE[(args.problem, args.dtype)]
+    peak = sw.measure_alu_peak(sw_dtype)["instr_per_s"]
+    achieved = fpi * stage_updates / t_diamond if fpi else None
+    roofline = {
+        "bound": "alu", "kernel": f"swept diamond ({'wave' if kernel == sw.KERNEL_WAVE else 'smem'}) W={W}",
+        "achieved": achieved / 1e12 if achieved else None, "peak": peak / 1e12, "unit": "T FP-instr/s (thread-level)",
+        "frac": (achieved / peak) if achieved else None, "traffic": None,
+        "peak_source": "measured FMA-chain microbenchmark (swept_measure_alu_peak), same process",
+        "launch_ms": t_diamond * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
+        "hbm_algorithmic_bytes_per_launch": int(4 * w.nx * sw.NCOMP[w.problem] * u.element_size()),
+    }
+
+    # ---- classic path on the same workload (context: swept / classic speedup) ------------------------------
+    classic = None
+    if not args.no_classic:
+        ns_naive = min(w.nsteps, 2000)
+        u.copy_(u0_host)
+        s.naive_run(u, ns_naive)
+        t_naive = timed(lambda: s.naive_run(u, ns_naive), 1)
+        naive_val = w.nx * ns_naive / t_naive / 1e9
+        s.set_option(sw.OPT_NAIVE_GRAPH, 1)
+        s.naive_run(u, ns_naive)
+        t_naive_g = timed(lambda: s.naive_run(u, ns_naive), 1)
+        naive_graph_val = w.nx * ns_naive / t_naive_g / 1e9
+        naive_bytes = {"heat": 2, "ks": 5, "euler": 15}[args.problem] * u.element_size()
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+            hbm_src = "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+        classic = {"value": naive_val, "value_graph": naive_graph_val, "unit": "GPts*steps/s", "timesteps": ns_naive,
+                   "algorithmic_GBps": naive_val * naive_bytes, "algorithmic_GBps_graph": naive_graph_val * naive_bytes,
+                   "hbm_peak_GBps": hbm_peak, "hbm_peak_source": hbm_src,
+                   "frac_of_hbm": max(naive_val, naive_graph_val) * naive_bytes / hbm_peak,
+                   "note": "fields up to nx=2^22 are L2-resident, so the classic path can exceed the HBM figure",
+                   "speedup_swept_over_classic": value / world / max(naive_val, naive_graph_val)}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        rate, n, el, cores = oracle_rate(w, np_dtype)
+        cpu = {"value": rate / 1e9, "unit": "GPts*steps/s", "cores": cores, "kind": "oracle",
+               "sample": f"{n} of {w.nsteps} timesteps at nx={w.nx} ({el:.1f} s)"}
+
+    out = {
+        "metric": "grid-point updates/sec", "value": value, "unit": "GPts*steps/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": t_dev_max / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {
+            "workload": f"BASELINE.json configs[1]: {w.name}, FTCS periodic r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
+                        f"{w.nsteps} timesteps per step" if args.problem == "heat" else f"{w.name} nx={w.nx} {w.nsteps} timesteps per step",
+            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": args.kernel if kernel == sw.KERNEL_WAVE else "smem",
+            "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
+        },
+        "e2e": {"value": e2e_value, "unit": "GPts*steps/s", "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes},
+        "gpu_launches": int(launches),
+        "clocks": clk.summary(),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "classic": classic,
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
