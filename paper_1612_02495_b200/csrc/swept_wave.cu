@@ -1,7 +1,49 @@
-// swept_wave.cu -- placeholder until the register-resident wavefront kernels land.
+// swept_wave.cu -- problem dispatch for the wavefront swept kernels (instantiated in swept_wave_<problem>.cu).
 #include "internal.h"
+
 namespace swept {
-cudaError_t launch_swept_wave(int, int, int, void *, void *, int64_t, int, int64_t, const ConstBlock &, int, int, cudaStream_t) { return cudaErrorNotSupported; }
-int swept_wave_supports(int, int, int) { return 0; }
-cudaError_t swept_wave_prepare(int, int) { return cudaSuccess; }
+
+#define DECL(prob)                                                                                                              \
+    cudaError_t launch_swept_wave_##prob(int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,              \
+                                         const ConstBlock &cb, int wpb, size_t smem_floor, cudaStream_t st);                    \
+    cudaError_t swept_wave_prepare_##prob(int dtype, int max_smem);                                                             \
+    int swept_wave_supports_##prob(int W);
+DECL(heat)
+DECL(ks)
+DECL(euler)
+#undef DECL
+
+// Shared memory request that caps resident blocks per SM at `cap` (SWEPT_OPT_BLOCKS_PER_SM): each block is charged its
+// request plus 1 KB of system use against the SM's 228 KB.
+size_t smem_floor_for_cap(int cap) {
+    if (cap <= 0) return 0;
+    const size_t total = 228 * 1024, sys = 1024, limit = 227 * 1024;
+    size_t req = total / (size_t)cap - sys;
+    return req > limit ? limit : req;
 }
+
+cudaError_t launch_swept_wave(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
+                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, cudaStream_t st) {
+    const size_t floor = smem_floor_for_cap(blocks_per_sm);
+    if (problem == SWEPT_HEAT) return launch_swept_wave_heat(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
+    if (problem == SWEPT_KS) return launch_swept_wave_ks(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
+    return launch_swept_wave_euler(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
+}
+
+int swept_wave_supports(int problem, int dtype, int W) {
+    (void)dtype;
+    if (problem == SWEPT_HEAT) return swept_wave_supports_heat(W);
+    if (problem == SWEPT_KS) return swept_wave_supports_ks(W);
+    return swept_wave_supports_euler(W);
+}
+
+cudaError_t swept_wave_prepare(int problem, int dtype) {
+    int dev = 0, max_smem = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (problem == SWEPT_HEAT) return swept_wave_prepare_heat(dtype, max_smem);
+    if (problem == SWEPT_KS) return swept_wave_prepare_ks(dtype, max_smem);
+    return swept_wave_prepare_euler(dtype, max_smem);
+}
+
+}  // namespace swept

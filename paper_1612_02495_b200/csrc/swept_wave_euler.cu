@@ -1,0 +1,31 @@
+// swept_wave_euler.cu -- instantiations of the wavefront swept kernels (swept_wave.cuh) for the euler problem.
+#include "swept_wave.cuh"
+namespace swept {
+template <class T> static cudaError_t launch_t(int mode, void *u, void *w, int64_t nx, int W, int64_t offset, const ConstBlock &cb, int wpb, size_t smem_floor, cudaStream_t st) {
+    switch (W / 32) {
+        case 4: return wave_launch_pw<Euler<T>, 4>(mode, u, w, nx, offset, cb, wpb, smem_floor, st);
+        case 8: return wave_launch_pw<Euler<T>, 8>(mode, u, w, nx, offset, cb, wpb, smem_floor, st);
+        case 16: return wave_launch_pw<Euler<T>, 16>(mode, u, w, nx, offset, cb, wpb, smem_floor, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+template <class T> static cudaError_t prepare_t(int max_smem) {
+    cudaError_t e = cudaSuccess;
+    if ((e = wave_prepare_pw<Euler<T>, 4>(max_smem)) != cudaSuccess) return e;
+    if ((e = wave_prepare_pw<Euler<T>, 8>(max_smem)) != cudaSuccess) return e;
+    if ((e = wave_prepare_pw<Euler<T>, 16>(max_smem)) != cudaSuccess) return e;
+    return e;
+}
+cudaError_t launch_swept_wave_euler(int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset, const ConstBlock &cb, int wpb, size_t smem_floor, cudaStream_t st) {
+    return dtype == SWEPT_F64 ? launch_t<double>(mode, u, w, nx, W, offset, cb, wpb, smem_floor, st) : launch_t<float>(mode, u, w, nx, W, offset, cb, wpb, smem_floor, st);
+}
+cudaError_t swept_wave_prepare_euler(int dtype, int max_smem) { return dtype == SWEPT_F64 ? prepare_t<double>(max_smem) : prepare_t<float>(max_smem); }
+int swept_wave_supports_euler(int W) {
+    switch (W) {
+        case 128: return 1;
+        case 256: return 1;
+        case 512: return 1;
+        default: return 0;
+    }
+}
+}  // namespace swept
