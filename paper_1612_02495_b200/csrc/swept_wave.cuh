@@ -89,40 +89,51 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
 #pragma unroll
                 for (int d = 0; d < D; ++d) feed[k][d] = io[k * W + fj + d];
         }
+        // Lane l-1's newest value of row rho is its column PW-D+r (r = D-1-rho), last written one super-row ago and not
+        // yet overwritten, so all D row inputs can be fetched before any of this super-row's updates.
+        T recv[NC][D];
 #pragma unroll
-        for (int rho = 0; rho < D; ++rho) {
-            const int r = D - 1 - rho;                // lattice residue of row j = D J + rho
-            T recv[NC];
+        for (int rho = 0; rho < D; ++rho)
 #pragma unroll
             for (int k = 0; k < NC; ++k) {
-                recv[k] = shfl_up1(X[k][PW + r]);     // lane l-1's newest value of this row (its column PW-D+r)
-                if (MODE != MODE_UP) recv[k] = (lane == 0) ? feed[k][rho] : recv[k];
+                recv[k][rho] = shfl_up1(X[k][PW + (D - 1 - rho)]);
+                if (MODE != MODE_UP) recv[k][rho] = (lane == 0) ? feed[k][rho] : recv[k][rho];
             }
-            if (act) {
-                T old[NC];
+        if (act) {
+            // Point n of row rho reads this super-row's point n-1 of rows <= rho and the previous super-row's values of
+            // the columns rows > rho will write at point n: looping n outside, rho inside keeps the in-place update
+            // correct and leaves the D points of one n independent of each other (instruction-level parallelism D).
+            T old[D][NC];
 #pragma unroll
-                for (int k = 0; k < NC; ++k) { old[k] = X[k][r]; X[k][r] = recv[k]; }
+            for (int rho = 0; rho < D; ++rho)
 #pragma unroll
-                for (int n = 0; n < NP; ++n) {
-                    const int q = r + D * n;          // window X[k][q .. q+D], target X[k][q+D]
+                for (int k = 0; k < NC; ++k) { old[rho][k] = X[k][D - 1 - rho]; X[k][D - 1 - rho] = recv[k][rho]; }
+#pragma unroll
+            for (int n = 0; n < NP; ++n) {
+                const int t = tb + n;
+                const bool odd = (t & 1) != 0;
+                const bool pact = (MODE == MODE_DIAMOND) ? true : (MODE == MODE_UP ? (t > L) : (t <= L));
+#pragma unroll
+                for (int rho = 0; rho < D; ++rho) {
+                    const int q = (D - 1 - rho) + D * n;   // row residue r = D-1-rho; window X[k][q .. q+D], target X[k][q+D]
                     T win[NC][2 * H + 1], out[NC];
 #pragma unroll
                     for (int k = 0; k < NC; ++k)
 #pragma unroll
                         for (int m = 0; m <= D; ++m) win[k][m] = X[k][q + m];
-                    const int t = tb + n;
-                    P::stage_sel(c, (t & 1) != 0, win, old, out);
-                    const bool pact = (MODE == MODE_DIAMOND) ? true : (MODE == MODE_UP ? (t > L) : (t <= L));
+                    P::stage_sel(c, odd, win, old[rho], out);
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
-                        old[k] = X[k][q + D];
+                        old[rho][k] = X[k][q + D];
                         X[k][q + D] = pact ? out[k] : X[k][q + D];
                     }
                 }
-                if (MODE != MODE_DOWN && lane == 31) {
+            }
+            if (MODE != MODE_DOWN && lane == 31) {    // the row outputs: newest value of row rho is column PW-D+r
 #pragma unroll
-                    for (int k = 0; k < NC; ++k) io[k * W + J * D + rho] = X[k][PW + r];
-                }
+                for (int k = 0; k < NC; ++k)
+#pragma unroll
+                    for (int rho = 0; rho < D; ++rho) io[k * W + J * D + rho] = X[k][PW + (D - 1 - rho)];
             }
         }
     }
