@@ -81,7 +81,7 @@ class ClockSampler:
                     self.rows.append([c.strip() for c in out.split(",")])
             except Exception:
                 pass
-            self._stop.wait(0.2)
+            self._stop.wait(0.05)
 
     def __enter__(self):
         self._t = threading.Thread(target=self._run, daemon=True)
@@ -109,13 +109,14 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------
 # CPU baseline / reference arm: the oracle as it stands, on the host cores, bounded sample
 # ---------------------------------------------------------------------------------------------------------------
-def oracle_rate(w: wl.Workload, dtype, budget_s: float = 12.0):
+def oracle_rate(w: wl.Workload, dtype, budget_s: float = 15.0):
     import oracle
     u0 = w.initial(dtype)
+    oracle.run(w.problem, u0, 2, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)      # thread start-up, page faults
     t0 = time.perf_counter()
-    oracle.run(w.problem, u0, 4, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
-    t4 = time.perf_counter() - t0
-    n = int(max(8, min(w.nsteps, budget_s / max(t4 / 4, 1e-9))))
+    oracle.run(w.problem, u0, 8, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    t8 = time.perf_counter() - t0
+    n = int(max(8, min(w.nsteps, budget_s / max(t8 / 8, 1e-9))))
     t0 = time.perf_counter()
     oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
     dt = time.perf_counter() - t0
@@ -157,10 +158,86 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------------------------
+# --sweep: the paper's experiment E1/E2 (Fig. 8-9) re-measured on B200 -- for every nx of the config's
+# range, every legal tile width against the classic path, best width kept.
+# ---------------------------------------------------------------------------------------------------------------
+SWEEP_NX = {"heat": range(11, 23), "ks": range(14, 21), "euler": range(12, 21)}
+
+
+def run_sweep(args):
+    import torch
+
+    import paper_1612_02495_b200 as sw
+
+    torch.cuda.set_device(0)
+    np_dtype = np.float64 if args.dtype == "f64" else np.float32
+    sw_dtype = sw.F64 if args.dtype == "f64" else sw.F32
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, reps=3):
+        fn()                                   # warm-up (also builds a graph on first use)
+        ts = []
+        for _ in range(reps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream); e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        return statistics.median(ts)
+
+    rows = []
+    for lg in SWEEP_NX[args.problem]:
+        nx = 1 << lg
+        w = wl.make(args.problem, nx, "config")
+        if args.nsteps:
+            w.nsteps = args.nsteps
+        u0 = torch.from_numpy(w.initial(np_dtype)).cuda()
+        u = u0.clone()
+        row = {"nx": nx, "log2_nx": lg, "nsteps": w.nsteps, "swept": {}}
+        with sw.Solver(w.problem, nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma) as s:
+            ns_naive = min(w.nsteps, 2000)
+            t = timed(lambda: s.naive_run(u, ns_naive))
+            row["naive"] = nx * ns_naive / t / 1e9
+            s.set_option(sw.OPT_NAIVE_GRAPH, 1)
+            t = timed(lambda: s.naive_run(u, ns_naive))
+            row["naive_graph"] = nx * ns_naive / t / 1e9
+            for kname, kid in (("wave", sw.KERNEL_WAVE), ("smem", sw.KERNEL_SMEM)):
+                s.set_option(sw.OPT_KERNEL, kid)
+                for W in (32, 64, 128, 256, 512, 1024, 2048):
+                    if W > nx or not s.tile_width_ok(W):
+                        continue
+                    for graph in (0, 1):
+                        s.set_option(sw.OPT_SWEPT_GRAPH, graph)
+                        u.copy_(u0)
+                        t = timed(lambda: s.swept_run(u, w.nsteps, W), reps=3 if nx <= (1 << 20) else 2)
+                        row["swept"][f"{kname}/W={W}/{'graph' if graph else 'plain'}"] = nx * w.nsteps / t / 1e9
+        best = max(row["swept"], key=row["swept"].get)
+        row["best"], row["best_value"] = best, row["swept"][best]
+        best_paper = max((k for k in row["swept"] if k.startswith("smem") and k.endswith("plain")), key=row["swept"].get)
+        row["best_paper_style"], row["best_paper_style_value"] = best_paper, row["swept"][best_paper]
+        row["speedup_vs_naive"] = row["best_value"] / row["naive"]
+        row["speedup_vs_naive_graph"] = row["best_value"] / row["naive_graph"]
+        rows.append(row)
+        print(f"# nx=2^{lg}: naive {row['naive']:.2f} (graph {row['naive_graph']:.2f})  best swept {best} {row['best_value']:.1f} "
+              f"GPts*steps/s  x{row['speedup_vs_naive']:.1f} / x{row['speedup_vs_naive_graph']:.1f}", file=sys.stderr, flush=True)
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    out = {"problem": args.problem, "dtype": args.dtype, "unit": "GPts*steps/s", "rows": rows}
+    with open(os.path.join(ROOT, "gpurun_out", f"sweep_{args.problem}_{args.dtype}.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print(f"| nx | classic (plain launches) | classic (graph) | paper-style swept (smem, plain) | best swept | config | speedup vs classic | vs classic graph |")
+    print("|---|---:|---:|---:|---:|---|---:|---:|")
+    for r in rows:
+        print(f"| 2^{r['log2_nx']} | {r['naive']:.2f} | {r['naive_graph']:.2f} | {r['best_paper_style_value']:.1f} ({r['best_paper_style'].split('/')[1]}) | "
+              f"{r['best_value']:.1f} | {r['best']} | {r['speedup_vs_naive']:.1f}x | {r['speedup_vs_naive_graph']:.1f}x |")
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.sweep:
+        run_sweep(args)
         return
 
     import torch
