@@ -57,8 +57,30 @@ enum {
                                      plain launches = the paper's classic program)               */
     SWEPT_OPT_BLOCKS_PER_SM = 2,  /* cap on resident blocks per SM for the swept kernels, 0 = none */
     SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
-    SWEPT_OPT_SWEPT_GRAPH = 4     /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
+    SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
+    SWEPT_OPT_CHAIN = 5           /* WAVE kernels: 1 (default) = launch-free sweep, ONE persistent launch runs all
+                                     half-cycles of a swept_run, tiles ordered by per-tile flags in global memory
+                                     (beyond the paper; removes PAPER.md:232's launch/wave costs); 0 = one launch
+                                     per half-cycle as in the paper                   */
 };
+
+/* Shared memory a block may opt in to on B200 (227 KB); swept_plan, which has no device, checks SMEM-kernel tile widths
+ * against it (a handle checks against the device's own attribute). */
+#define SWEPT_SMEM_LIMIT_B200 232448
+
+/* One entry of the launch plan of swept_run (host driver):
+ *   CLASSIC  `count` classic timesteps (count * S kernels)
+ *   UP       upright triangles, tiles at `offset`                                  (Fig. 5)
+ *   DIAMOND  `count` consecutive diamond launches, the first at `offset`, then alternating 0 <-> W/2
+ *   DOWN     closing inverted triangles at `offset`
+ *   CHAIN    `count` half-cycles (1 UP + (count-1) DIAMOND + 1 DOWN phases, offsets 0, W/2, 0, ...) in ONE launch */
+enum { SWEPT_LAUNCH_CLASSIC = 0, SWEPT_LAUNCH_UP = 1, SWEPT_LAUNCH_DIAMOND = 2, SWEPT_LAUNCH_DOWN = 3, SWEPT_LAUNCH_CHAIN = 4 };
+typedef struct {
+    int kind;           /* SWEPT_LAUNCH_*                         */
+    int tile_width;     /* W of the entry (0 for CLASSIC)         */
+    int64_t offset;     /* tile-grid shift of the (first) launch  */
+    int64_t count;      /* see above                              */
+} swept_launch_t;
 
 typedef struct {
     int dtype;          /* SWEPT_F32 | SWEPT_F64                                               */
@@ -106,6 +128,15 @@ int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void 
  * out (heat ping-pongs d_u and the workspace; two-stage schemes write the predictor to the
  * workspace and accumulate the final stage onto d_u, Fig. 6 `+=`).  Same argument rules as swept_run. */
 int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
+
+/* The launch list swept_run(h, d_u, nsteps, tile_width) enqueues for a solver of (problem, dtype, nx) with the given
+ * kernel family (SWEPT_KERNEL_*) and chain option: host logic only, needs neither a handle nor a device.  Writes up
+ * to `cap` entries to out (may be NULL when cap == 0) and returns the number of entries of the full plan, or a negative
+ * error code (illegal width, bad arguments).  Reading S3 of DESIGN.md: with nsteps = q*(L/S) + r, the r remainder
+ * timesteps come first -- one UP + DOWN pair on each narrower legal width of r's binary decomposition, then CLASSIC for
+ * what is left -- followed by the q half-cycles of width tile_width. */
+int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int tile_width, int kernel, int chain,
+                   swept_launch_t *out, int64_t cap);
 
 /* The paper's best-node-size sweep: time swept_run on d_u_scratch (device,
  * [ncomp][nx], contents destroyed) for every legal tile width (and kernel launch shape) up to

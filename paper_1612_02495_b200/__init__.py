@@ -18,7 +18,9 @@ from typing import Optional
 HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
-OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH = 0, 1, 2, 3, 4
+OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN = 0, 1, 2, 3, 4, 5
+LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN = 0, 1, 2, 3, 4
+LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain"}
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
 RADIUS = {HEAT: 1, KS: 2, EULER: 2}
@@ -28,7 +30,7 @@ NCOMP = {HEAT: 1, KS: 1, EULER: 3}
 # every symbol include/swept1d.h declares
 SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
-    "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version",
+    "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -52,6 +54,10 @@ class _Info(ctypes.Structure):
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
         ("max_smem_per_block", ctypes.c_int),
     ]
+
+
+class _Launch(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int), ("tile_width", ctypes.c_int), ("offset", ctypes.c_int64), ("count", ctypes.c_int64)]
 
 
 _lib = None
@@ -84,8 +90,10 @@ def lib() -> ctypes.CDLL:
     L.swept_tile_width_ok.argtypes = [vp, ci]
     L.swept_measure_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     L.swept_destroy.argtypes = [vp]
+    L.swept_plan.argtypes = [ci, ci, i64, i64, ci, ci, ci, ctypes.POINTER(_Launch), i64]
     for name in SYMBOLS:
         getattr(L, name).restype = ci
+    L.swept_plan.restype = i64
     L.swept_last_error.restype = ctypes.c_char_p
     L.swept_last_error.argtypes = []
     L.swept_version.restype = ctypes.c_char_p
@@ -205,6 +213,15 @@ def measure_alu_peak(dtype=F64, stream=None) -> dict:
     ips, ms = ctypes.c_double(0), ctypes.c_double(0)
     _check(lib().swept_measure_alu_peak(_dtype_id(dtype), ctypes.byref(ips), ctypes.byref(ms), _stream_ptr(stream)))
     return {"instr_per_s": ips.value, "ms": ms.value}
+
+
+def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: bool = True) -> list:
+    """The launch list `swept_run` enqueues (swept_plan; host logic, no device needed): [(kind, W, offset, count), ...]."""
+    buf = (_Launch * 64)()
+    n = lib().swept_plan(int(problem), int(dtype), int(nx), int(nsteps), int(tile_width), int(kernel), int(bool(chain)), buf, 64)
+    if n < 0:
+        _check(int(n))
+    return [(buf[i].kind, buf[i].tile_width, buf[i].offset, buf[i].count) for i in range(min(int(n), 64))]
 
 
 def steps_per_half_cycle(problem: int, tile_width: int) -> int:

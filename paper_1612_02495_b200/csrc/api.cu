@@ -22,12 +22,13 @@ struct swept_ctx {
     size_t field_bytes;    // NC*nx*sizeof(T)
     void *host_stage;      // device buffer for swept_run_host (allocated on first use)
     int device, sm_count, max_smem;
-    int kernel, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
+    int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
+    void *sync;            // chain kernel: work counter (8 bytes) + done[nx / 8] flags
     int max_tile_width, tuned_tile_width;
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
-    cudaGraphExec_t sgraph;  void *sgraph_u;  int64_t sgraph_steps;  int sgraph_W, sgraph_kernel;
+    cudaGraphExec_t sgraph;  void *sgraph_u;  int64_t sgraph_steps;  int sgraph_W, sgraph_kernel, sgraph_chain;
     int64_t sgraph_launches;
 };
 
@@ -106,6 +107,7 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     h->nx = nx; h->dx = dx; h->dt = dt; h->alpha = alpha; h->gamma = gamma;
     h->device = dev;
     h->kernel = SWEPT_KERNEL_WAVE;
+    h->chain = 1;
     h->warps_per_block = 4;
     h->max_tile_width = p ? p->max_tile_width : 0;
     if (dtype == SWEPT_F64) fill_consts<double>(h); else fill_consts<float>(h);
@@ -118,9 +120,16 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
         cudaGetLastError();
         return fail(e == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "swept_create: cudaMalloc workspace: %s", cudaGetErrorString(e));
     }
+    e = cudaMalloc(&h->sync, 8 + sizeof(unsigned) * (size_t)(nx / 8));
+    if (e != cudaSuccess) {
+        cudaFree(h->work);
+        delete h;
+        cudaGetLastError();
+        return fail(e == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "swept_create: cudaMalloc flags: %s", cudaGetErrorString(e));
+    }
     e = swept_smem_prepare(problem, dtype, (size_t)h->max_smem);
     if (e == cudaSuccess) e = swept_wave_prepare(problem, dtype);
-    if (e != cudaSuccess) { cudaFree(h->work); delete h; return fail_cuda(e, "swept_create: kernel attribute setup"); }
+    if (e != cudaSuccess) { cudaFree(h->work); cudaFree(h->sync); delete h; return fail_cuda(e, "swept_create: kernel attribute setup"); }
     *out = h;
     return SWEPT_OK;
 }
@@ -134,27 +143,33 @@ extern "C" int swept_destroy(swept_handle_t h) {
     if (!h) return fail(SWEPT_EINVAL, "swept_destroy: NULL handle");
     drop_graphs(h);
     if (h->work) cudaFree(h->work);
+    if (h->sync) cudaFree(h->sync);
     if (h->host_stage) cudaFree(h->host_stage);
     delete h;
     return SWEPT_OK;
 }
 
 // ---- legality of a tile width (SURVEY.md section 8(a) "Legal tile widths") ------------------------------------
-static int check_width(const swept_ctx *h, int W, int kernel, bool set_err) {
-    const char *why = nullptr;
-    char buf[160];
-    if (W <= 0 || !is_pow2(W)) why = "tile width must be a power of two";
-    else if (W < 4 * h->H) why = "tile width must be >= 4h (L = W/(2h) even)";
-    else if ((int64_t)W > h->nx) why = "tile width exceeds nx";
-    else if (kernel == SWEPT_KERNEL_SMEM) {
-        const size_t need = swept_smem_bytes(h->problem, h->dtype, W);
-        if (need > (size_t)h->max_smem) {
-            snprintf(buf, sizeof buf, "tile needs %zu B of shared memory, limit %d B", need, h->max_smem);
-            why = buf;
+static const char *width_problem(int problem, int dtype, int64_t nx, int W, int kernel, int max_smem, char *buf, size_t nbuf) {
+    const int H = radius_of(problem);
+    if (W <= 0 || !is_pow2(W)) return "tile width must be a power of two";
+    if (W < 4 * H) return "tile width must be >= 4h (L = W/(2h) even)";
+    if ((int64_t)W > nx) return "tile width exceeds nx";
+    if (kernel == SWEPT_KERNEL_SMEM) {
+        const size_t need = swept_smem_bytes(problem, dtype, W);
+        if (need > (size_t)max_smem) {
+            snprintf(buf, nbuf, "tile needs %zu B of shared memory, limit %d B", need, max_smem);
+            return buf;
         }
-    } else if (kernel == SWEPT_KERNEL_WAVE) {
-        if (!swept_wave_supports(h->problem, h->dtype, W)) why = "tile width not supported by the WAVE kernels for this problem/dtype";
-    } else why = "unknown kernel";
+        return nullptr;
+    }
+    if (kernel == SWEPT_KERNEL_WAVE) return swept_wave_supports(problem, dtype, W) ? nullptr : "tile width not supported by the WAVE kernels for this problem/dtype";
+    return "unknown kernel";
+}
+
+static int check_width(const swept_ctx *h, int W, int kernel, bool set_err) {
+    char buf[160];
+    const char *why = width_problem(h->problem, h->dtype, h->nx, W, kernel, h->max_smem, buf, sizeof buf);
     if (why) {
         if (set_err) fail(SWEPT_EINVAL, "tile_width %d: %s", W, why);
         return 0;
@@ -189,8 +204,7 @@ static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cuda
             ++*launches;
         }
         if (a != d_u) {
-            e = cudaMemcpyAsync(d_u, a, h->field_bytes, cudaMemcpyDeviceToDevice, st);
-            ++*launches;
+            e = cudaMemcpyAsync(d_u, a, h->field_bytes, cudaMemcpyDeviceToDevice, st);   // a copy, not a kernel: not counted
         }
     } else {
         for (int64_t m = 0; m < nsteps; ++m) {
@@ -269,47 +283,89 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
 }
 
 // ---- swept path (row A7) ---------------------------------------------------------------------------------------
+// The host driver is data: build_plan() turns (nsteps, W) into the launch list, enqueue_plan() executes it.
+// nsteps = q*(L/S) + r.  The r remaining timesteps run first (reading S3): on successively narrower legal tiles (each
+// one half-cycle: one upright + one closing triangle), and what no tile width divides on the classic kernel.  Then q
+// half-cycles of width W: 1 upright triangle + (q-1) diamonds on tiles shifted by W/2 each launch + 1 closing inverted
+// triangle; on a periodic domain either alignment may write out (reading S4).  With `chain` (WAVE
+// kernels) the q half-cycles are ONE launch of the flag-ordered persistent kernel.
+static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int W, int kernel, int chain, int max_smem,
+                          swept_launch_t *out, int64_t cap) {
+    const int H = radius_of(problem), S = stages_of(problem);
+    const int per = 2 * H * S;   // W / per = timesteps per half-cycle
+    int64_t n = 0;
+    auto push = [&](int kind, int w, int64_t offset, int64_t count) {
+        if (out && n < cap) { out[n].kind = kind; out[n].tile_width = w; out[n].offset = offset; out[n].count = count; }
+        ++n;
+    };
+    auto half_cycles = [&](int w, int64_t q, bool chained) {
+        if (q <= 0) return;
+        if (chained) { push(SWEPT_LAUNCH_CHAIN, w, 0, q); return; }
+        push(SWEPT_LAUNCH_UP, w, 0, 1);
+        if (q > 1) push(SWEPT_LAUNCH_DIAMOND, w, w / 2, q - 1);   // offsets W/2, 0, W/2, ...
+        push(SWEPT_LAUNCH_DOWN, w, (q & 1) ? w / 2 : 0, 1);
+    };
+    const int64_t sph = W / per;
+    const int64_t q = nsteps / sph;
+    int64_t r = nsteps % sph;
+    char buf[160];
+    for (int w = W / 2; w >= 4 * H && r > 0; w >>= 1) {
+        const int64_t s = w / per;
+        if (s >= 1 && r >= s && !width_problem(problem, dtype, nx, w, kernel, max_smem, buf, sizeof buf)) {
+            half_cycles(w, 1, false);
+            r -= s;
+        }
+    }
+    if (r > 0) push(SWEPT_LAUNCH_CLASSIC, 0, 0, r);
+    half_cycles(W, q, chain && kernel == SWEPT_KERNEL_WAVE);
+    return n;
+}
+
+extern "C" int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int tile_width, int kernel, int chain,
+                              swept_launch_t *out, int64_t cap) {
+    if (problem != SWEPT_HEAT && problem != SWEPT_KS && problem != SWEPT_EULER) return fail(SWEPT_EINVAL, "swept_plan: unknown problem %d", problem);
+    if (dtype != SWEPT_F32 && dtype != SWEPT_F64) return fail(SWEPT_EINVAL, "swept_plan: unknown dtype %d", dtype);
+    if (!is_pow2(nx) || nx < 8) return fail(SWEPT_EINVAL, "swept_plan: nx=%lld must be a power of two >= 8", (long long)nx);
+    if (nsteps < 0) return fail(SWEPT_EINVAL, "swept_plan: nsteps < 0");
+    if (cap < 0 || (cap > 0 && !out)) return fail(SWEPT_EINVAL, "swept_plan: bad output buffer");
+    char buf[160];
+    const char *why = width_problem(problem, dtype, nx, tile_width, kernel, SWEPT_SMEM_LIMIT_B200, buf, sizeof buf);
+    if (why) return fail(SWEPT_EINVAL, "tile_width %d: %s", tile_width, why);
+    return build_plan(problem, dtype, nx, nsteps, tile_width, kernel, chain, SWEPT_SMEM_LIMIT_B200, out, cap);
+}
+
 static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, int W, int64_t offset, cudaStream_t st) {
     if (kernel == SWEPT_KERNEL_SMEM) return launch_swept_smem(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, st);
     return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, h->blocks_per_sm, st);
 }
 
-// q half-cycles of width W: 1 upright triangle + (q-1) diamonds on tiles shifted by W/2 each launch + 1 closing
-// inverted triangle.  On a periodic domain either alignment may write out (reading S4).
-static cudaError_t enqueue_half_cycles(swept_ctx *h, int kernel, void *d_u, int W, int64_t q, cudaStream_t st, int64_t *launches) {
-    if (q <= 0) return cudaSuccess;
-    cudaError_t e = launch_phase(h, kernel, MODE_UP, d_u, W, 0, st);
-    if (e != cudaSuccess) return e;
-    for (int64_t i = 1; i < q; ++i) {
-        e = launch_phase(h, kernel, MODE_DIAMOND, d_u, W, (i & 1) ? W / 2 : 0, st);
-        if (e != cudaSuccess) return e;
-    }
-    e = launch_phase(h, kernel, MODE_DOWN, d_u, W, (q & 1) ? W / 2 : 0, st);
-    *launches += q + 1;
-    return e;
-}
-
-// nsteps = q*(L/S) + r.  The r remaining timesteps run first (reading S3): on successively narrower legal tiles
-// (each one half-cycle: one upright + one closing triangle), and what no tile width divides on the classic kernel.
 static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches) {
-    const int per = 2 * h->H * h->S;   // W / per = timesteps per half-cycle
-    const int64_t sph = W / per;
-    const int64_t q = nsteps / sph;
-    int64_t r = nsteps % sph;
+    swept_launch_t plan[64];   // at most 3 entries per narrower width + 1 classic + 3
+    const int64_t n = build_plan(h->problem, h->dtype, h->nx, nsteps, W, kernel, h->chain, h->max_smem, plan, 64);
+    if (n > 64) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
-    for (int w = W / 2; w >= 4 * h->H && r > 0; w >>= 1) {
-        const int64_t s = w / per;
-        if (s >= 1 && r >= s && check_width(h, w, kernel, false)) {
-            e = enqueue_half_cycles(h, kernel, d_u, w, 1, st, launches);
-            if (e != cudaSuccess) return e;
-            r -= s;
+    for (int64_t i = 0; i < n && e == cudaSuccess; ++i) {
+        const swept_launch_t &L = plan[i];
+        switch (L.kind) {
+            case SWEPT_LAUNCH_CLASSIC: e = enqueue_classic(h, d_u, L.count, st, launches); break;
+            case SWEPT_LAUNCH_UP: e = launch_phase(h, kernel, MODE_UP, d_u, L.tile_width, L.offset, st); ++*launches; break;
+            case SWEPT_LAUNCH_DOWN: e = launch_phase(h, kernel, MODE_DOWN, d_u, L.tile_width, L.offset, st); ++*launches; break;
+            case SWEPT_LAUNCH_DIAMOND:
+                for (int64_t k = 0; k < L.count && e == cudaSuccess; ++k) {
+                    const int64_t off = (k & 1) ? (L.offset ? 0 : L.tile_width / 2) : L.offset;
+                    e = launch_phase(h, kernel, MODE_DIAMOND, d_u, L.tile_width, off, st);
+                    ++*launches;
+                }
+                break;
+            case SWEPT_LAUNCH_CHAIN:
+                e = launch_swept_chain(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->warps_per_block,
+                                       h->blocks_per_sm, h->sm_count, st);
+                ++*launches;
+                break;
+            default: e = cudaErrorInvalidValue;
         }
     }
-    if (r > 0) {
-        e = enqueue_classic(h, d_u, r, st, launches);
-        if (e != cudaSuccess) return e;
-    }
-    return enqueue_half_cycles(h, kernel, d_u, W, q, st, launches);
+    return e;
 }
 
 extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void *cuda_stream) {
@@ -323,11 +379,11 @@ extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_w
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int64_t launches = 0;
     if (h->swept_graph && nsteps > 0) {
-        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel;
+        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel && h->sgraph_chain == h->chain;
         int64_t l = 0;
         rc = run_graphed(&h->sgraph, reuse, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_swept(h, h->kernel, d_u, nsteps, W, s, n); }, "swept_run(graph)");
         if (rc) return rc;
-        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_launches = l; }
+        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_chain = h->chain; h->sgraph_launches = l; }
         launches = h->sgraph_launches;
     } else {
         cudaError_t e = enqueue_swept(h, h->kernel, d_u, nsteps, W, st, &launches);
@@ -423,6 +479,10 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
         case SWEPT_OPT_SWEPT_GRAPH:
             if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: SWEPT_GRAPH takes 0 or 1");
             h->swept_graph = value;
+            return SWEPT_OK;
+        case SWEPT_OPT_CHAIN:
+            if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0 or 1");
+            h->chain = value;
             return SWEPT_OK;
         case SWEPT_OPT_BLOCKS_PER_SM:
             if (value < 0 || value > 32) return fail(SWEPT_EINVAL, "swept_set_option: BLOCKS_PER_SM takes 0..32");

@@ -31,6 +31,10 @@ cudaError_t swept_smem_prepare(int problem, int dtype, size_t max_bytes);
 // Register-resident wavefront swept kernels (swept_wave.cu): one warp per tile of W points.
 cudaError_t launch_swept_wave(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
                               const ConstBlock &cb, int warps_per_block, int blocks_per_sm, cudaStream_t st);
+// Launch-free sweep: ONE launch runs q half-cycles (1 upright + (q-1) diamond + 1 closing phase), tiles ordered by per-tile
+// flags in `sync` (8 + 4*nx/W bytes, zeroed by the launch helper).
+cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
+                               int warps_per_block, int blocks_per_sm, int sm_count, cudaStream_t st);
 int swept_wave_supports(int problem, int dtype, int W);
 cudaError_t swept_wave_prepare(int problem, int dtype);
 

@@ -28,21 +28,21 @@ namespace swept {
 
 template <class T> __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
-template <class P, int PW, int MODE>
-__global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, typename P::real *w, int64_t nx, int64_t offset,
-                                                          int ntiles, typename P::Consts c) {
+// Staircase loads/stores.  CG = true (chained persistent kernel): cache at L2 only, because another SM may have
+// rewritten the line since this SM last read it (the flag acquire orders the accesses, .cg keeps L1 out of it).
+template <bool CG, class T> __device__ __forceinline__ T ld_stair(const T *p) { return CG ? __ldcg(p) : *p; }
+template <bool CG, class T> __device__ __forceinline__ void st_stair(T *p, T v) { if (CG) __stcg(p, v); else *p = v; }
+
+// One tile (one warp): g0 = global index of the tile's first point (before the periodic wrap), io = the warp's
+// shared-memory row buffer of NC*W values.
+template <class P, int PW, int MODE, bool CG>
+__device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real *w, const int64_t nx, const int64_t g0,
+                                          typename P::real *io, const typename P::Consts &c, const int lane) {
     using T = typename P::real;
     constexpr int H = P::H, NC = P::NC, D = 2 * H;
     constexpr int W = 32 * PW, NJ = W / D, NP = PW / D, L = W / D, CTR = W / 2;
     static_assert(PW % D == 0, "points per lane must be a multiple of 2H");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-
-    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
-    const int tile = (int)blockIdx.x * (int)(blockDim.x >> 5) + warp;
-    if (tile >= ntiles) return;                      // whole warps only
-    T *io = reinterpret_cast<T *>(smem_raw) + (size_t)warp * NC * W;   // io[k*W + j]: row feed in, right edge out
     const int64_t mask = nx - 1;
-    const int64_t g0 = (int64_t)tile * W + offset;
 
     // X[k][0..D) = copy of lane l-1's last D columns, X[k][D + q] = own column q
     T X[NC][D + PW];
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
 #pragma unroll
         for (int k = 0; k < NC; ++k)
 #pragma unroll
-            for (int q = 0; q < PW; ++q) X[k][D + q] = u[(int64_t)k * nx + ((g0 + lane * PW + q) & mask)];
+            for (int q = 0; q < PW; ++q) X[k][D + q] = ld_stair<CG>(u + (int64_t)k * nx + ((g0 + lane * PW + q) & mask));
     } else {
         // column i = 2H m + r starts from tier m of the right neighbour triangle's left edge: R_{m&1}[c + H m + r]
 #pragma unroll
@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
             const T *src = (m & 1) ? w : u;
             const int64_t g = (g0 + CTR + H * m + r) & mask;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) X[k][D + q] = src[(int64_t)k * nx + g];
+            for (int k = 0; k < NC; ++k) X[k][D + q] = ld_stair<CG>(src + (int64_t)k * nx + g);
         }
         // row j = 2H m + rho is fed from tier m of the left neighbour triangle's right edge: R_{m&1}[c - H m - rho - 1]
         for (int j = lane; j < W; j += 32) {
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
             const T *src = (m & 1) ? w : u;
             const int64_t g = (g0 + CTR - H * m - rho - 1) & mask;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) io[k * W + j] = src[(int64_t)k * nx + g];
+            for (int k = 0; k < NC; ++k) io[k * W + j] = ld_stair<CG>(src + (int64_t)k * nx + g);
         }
         __syncwarp();
     }
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
 #pragma unroll
         for (int k = 0; k < NC; ++k)
 #pragma unroll
-            for (int q = 0; q < PW; ++q) u[(int64_t)k * nx + ((g0 + lane * PW + q) & mask)] = X[k][D + q];
+            for (int q = 0; q < PW; ++q) st_stair<CG>(u + (int64_t)k * nx + ((g0 + lane * PW + q) & mask), X[k][D + q]);
     } else {
         // final column state: column i = 2H m + r holds tier L+m at x = H m + r  -> R_{m&1}[H m + r]
 #pragma unroll
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
             T *dst = (m & 1) ? w : u;
             const int64_t g = (g0 + H * m + r) & mask;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) dst[(int64_t)k * nx + g] = X[k][D + q];
+            for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, X[k][D + q]);
         }
         __syncwarp();
         // lane 31's row outputs: row j = 2H m + rho holds tier L+m at x = W-1-H m-rho -> R_{m&1}[W - 1 - H m - rho]
@@ -160,8 +160,80 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
             T *dst = (m & 1) ? w : u;
             const int64_t g = (g0 + W - 1 - H * m - rho) & mask;
 #pragma unroll
-            for (int k = 0; k < NC; ++k) dst[(int64_t)k * nx + g] = io[k * W + j];
+            for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, io[k * W + j]);
         }
+    }
+}
+
+// One launch per phase (SWEPT_OPT_CHAIN = 0): stream order between the launches is the only synchronisation.
+template <class P, int PW, int MODE>
+__global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, typename P::real *w, int64_t nx, int64_t offset,
+                                                          int ntiles, typename P::Consts c) {
+    using T = typename P::real;
+    constexpr int W = 32 * PW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    const int tile = (int)blockIdx.x * (int)(blockDim.x >> 5) + warp;
+    if (tile >= ntiles) return;                      // whole warps only
+    T *io = reinterpret_cast<T *>(smem_raw) + (size_t)warp * P::NC * W;   // io[k*W + j]: row feed in, right edge out
+    wave_tile<P, PW, MODE, false>(u, w, nx, (int64_t)tile * W + offset, io, c, lane);
+}
+
+// ---- launch-free sweep (SWEPT_OPT_CHAIN = 1, default) ----------------------------
+// ONE launch runs all q half-cycles: phase 0 = upright triangles (offset 0), phases 1..q-1 = diamonds (offset W/2, 0,
+// W/2, ...), phase q = closing inverted triangles.  Work items (phase, tile) are handed out in phase-major order by an
+// atomic counter; a warp that draws (p, t) waits until the two tiles of phase p-1 it stitches together (PAPER.md:86,
+// Fig. 2b: tile slots t and t+1 when phase p is the shifted one, t-1 and t otherwise) have published their staircases:
+// done[slot] = number of phases slot has completed (release store after the tile's last global store, acquire load
+// before the next tile's first global load).  Those two are the only tiles whose output (p, t) reads or overwrites
+// (DESIGN.md section 5.5), so no other ordering is needed, and because items are drawn in dependency order by warps
+// that are already running, the item with the smallest id in flight never waits: no co-residency requirement, no
+// grid-wide barrier.  Phase p+1 starts on the SMs that run out of phase-p tiles, so there is no tail between
+// half-cycles, and at small nx the cost of a kernel launch per half-cycle is gone.
+__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu(unsigned *p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <class P, int PW>
+__global__ void __launch_bounds__(256) swept_chain_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
+                                                           unsigned long long *counter, unsigned *done, typename P::Consts c) {
+    using T = typename P::real;
+    constexpr int W = 32 * PW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    T *io = reinterpret_cast<T *>(smem_raw) + (size_t)warp * P::NC * W;
+    const unsigned long long total = (unsigned long long)(q + 1) * (unsigned long long)ntiles;
+    for (;;) {
+        unsigned long long id = 0;
+        if (lane == 0) id = atomicAdd(counter, 1ull);
+        id = __shfl_sync(0xffffffffu, id, 0);
+        if (id >= total) break;
+        const int p = (int)(id / (unsigned long long)ntiles);
+        const int t = (int)(id - (unsigned long long)p * (unsigned long long)ntiles);
+        if (p > 0) {
+            if (lane < 2) {
+                int slot = t;
+                if (lane == 1) slot = (p & 1) ? (t + 1 == ntiles ? 0 : t + 1) : (t == 0 ? ntiles - 1 : t - 1);
+                unsigned ns = 20;
+                while (ld_acquire_gpu(done + slot) < (unsigned)p) {
+                    __nanosleep(ns);
+                    if (ns < 640) ns *= 2;
+                }
+            }
+            __syncwarp();
+        }
+        const int64_t g0 = (int64_t)t * W + ((p & 1) ? W / 2 : 0);
+        if (p == 0) wave_tile<P, PW, MODE_UP, true>(u, w, nx, g0, io, c, lane);
+        else if (p == q) wave_tile<P, PW, MODE_DOWN, true>(u, w, nx, g0, io, c, lane);
+        else wave_tile<P, PW, MODE_DIAMOND, true>(u, w, nx, g0, io, c, lane);
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) st_release_gpu(done + t, (unsigned)(p + 1));
     }
 }
 
@@ -184,8 +256,35 @@ cudaError_t wave_launch_pw(int mode, void *u, void *w, int64_t nx, int64_t offse
     return cudaGetLastError();
 }
 
+// Chain launch: grid = min(warps needed, resident warps) / wpb blocks; `sync` = counter (8 bytes) + done[ntiles] (zeroed here).
+template <class P, int PW>
+cudaError_t wave_chain_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count,
+                          cudaStream_t st) {
+    using T = typename P::real;
+    constexpr int W = 32 * PW;
+    const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
+    const int ntiles = (int)(nx / W);
+    if (wpb > 8) wpb = 8;
+    while (wpb > 1 && (int64_t)wpb * sm_count > ntiles) wpb >>= 1;   // few tiles: spread the warps over the SMs
+    size_t smem = (size_t)wpb * P::NC * W * sizeof(T);
+    if (smem < smem_floor) smem = smem_floor;
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, swept_chain_kernel<P, PW>, wpb * 32, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    int64_t blocks = (ntiles + wpb - 1) / wpb;
+    if (blocks > (int64_t)per_sm * sm_count) blocks = (int64_t)per_sm * sm_count;
+    e = cudaMemsetAsync(sync, 0, 8 + sizeof(unsigned) * (size_t)ntiles, st);
+    if (e != cudaSuccess) return e;
+    swept_chain_kernel<P, PW><<<(unsigned)blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, ntiles, (int)q, (unsigned long long *)sync,
+                                                                          (unsigned *)((char *)sync + 8), c);
+    return cudaGetLastError();
+}
+
 template <class P, int PW> cudaError_t wave_prepare_pw(int max_smem) {
-    cudaError_t e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_UP>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    cudaError_t e = cudaFuncSetAttribute(swept_chain_kernel<P, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_UP>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DIAMOND>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (e != cudaSuccess) return e;

@@ -31,10 +31,24 @@ def run_naive(w: wl.Workload, dtype, nsteps: int, u0=None, graph: bool = False) 
         return u.cpu().numpy()
 
 
-def run_swept(w: wl.Workload, dtype, nsteps: int, W: int, kernel: int, u0=None, graph: bool = False, opts=None) -> np.ndarray:
+# the swept kernel variants every parity test runs: (kernel family, chain option)
+SMEM, WAVE, CHAIN = (sw.KERNEL_SMEM, 0), (sw.KERNEL_WAVE, 0), (sw.KERNEL_WAVE, 1)
+VARIANTS = [SMEM, WAVE, CHAIN]
+VARIANT_IDS = ["smem", "wave", "chain"]
+
+
+def _select(s: sw.Solver, kernel) -> None:
+    if isinstance(kernel, tuple):
+        s.set_option(sw.OPT_KERNEL, kernel[0])
+        s.set_option(sw.OPT_CHAIN, kernel[1])
+    else:
+        s.set_option(sw.OPT_KERNEL, kernel)
+
+
+def run_swept(w: wl.Workload, dtype, nsteps: int, W: int, kernel, u0=None, graph: bool = False, opts=None) -> np.ndarray:
     import torch
     with solver_for(w, dtype) as s:
-        s.set_option(sw.OPT_KERNEL, kernel)
+        _select(s, kernel)
         if graph:
             s.set_option(sw.OPT_SWEPT_GRAPH, 1)
         for k, v in (opts or {}).items():
@@ -45,9 +59,9 @@ def run_swept(w: wl.Workload, dtype, nsteps: int, W: int, kernel: int, u0=None, 
         return u.cpu().numpy()
 
 
-def width_ok(w: wl.Workload, dtype, W: int, kernel: int) -> bool:
+def width_ok(w: wl.Workload, dtype, W: int, kernel) -> bool:
     with solver_for(w, dtype) as s:
-        s.set_option(sw.OPT_KERNEL, kernel)
+        _select(s, kernel)
         return s.tile_width_ok(W)
 
 

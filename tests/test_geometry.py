@@ -1,0 +1,202 @@
+"""-m "not gpu": the swept geometry and the host driver's launch plan, pinned to the
+numbers the paper prints (tests/golden/paper_geometry.txt) and to a plain-Python model of the swept rule.
+
+The model below restates PAPER.md:82-98, 102, 114 in the in-place staircase form of row A4: two flat rows R0 (even
+tiers) and R1 (odd tiers); a kernel of mode up / diamond / down loads R0 on [0,W) and R1 on [-h, W+h) of its tile,
+advances the tiers its mode prescribes with a plain periodic stencil, and stores R0 on [0,W), R1 on [h, W-h).  It is
+executed on the launch list `swept_plan` returns -- the very list `swept_run` enqueues -- and must reproduce naive
+stepping exactly (integer-valued stencils, so equality is exact), with every (point, tier) updated exactly once.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import paper_1612_02495_b200 as sw
+
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_geometry.txt")
+
+
+def _golden():
+    out = {}
+    for line in open(GOLDEN):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = int(line[1])
+    return out
+
+
+# ---- closed forms -----------------------------------------------------------------------
+def up_updates(W, h):
+    L = W // (2 * h)
+    return (L - 1) * W // 2
+
+
+def down_updates(W, h):
+    L = W // (2 * h)
+    return (L + 1) * W // 2
+
+
+def diamond_updates(W, h):
+    return (W // (2 * h)) * W
+
+
+def test_paper_geometry_numbers():
+    g = _golden()
+    n, h = 512, 1
+    # a full triangle (tier 0 included) for n = 512 holds 65 792 values = 514 kB in double
+    tri = sum(n - 2 * h * t for t in range(n // (2 * h)))
+    assert tri == g["triangle_values_n512"] == n + up_updates(n, h)
+    assert 8 * tri == g["triangle_bytes_n512_fp64"]
+    # the two-row matrix holds 2(n+2) values
+    assert 2 * (n + 2 * h) == g["two_row_values_n512"]
+    # a full cycle (two half-cycles) advances n timesteps for the heat scheme
+    assert 2 * sw.steps_per_half_cycle(sw.HEAT, n) == n * g["timesteps_per_cycle_heat_n"]
+    # a 32-point node gives four KS timesteps per (half-)cycle, "which only reduces instances of communication
+    # by 1/8": one global exchange per L = 8 sub-timesteps = 4 two-stage timesteps
+    assert sw.steps_per_half_cycle(sw.KS, 32) == g["ks_steps_per_cycle_n32"]
+    assert 32 // (2 * sw.RADIUS[sw.KS]) == 8
+
+
+def test_triangle_counts_sum_to_whole_tiers():
+    for h in (1, 2):
+        for W in (8, 32, 64, 512, 1024):
+            L = W // (2 * h)
+            assert up_updates(W, h) + down_updates(W, h) == diamond_updates(W, h) == L * W
+            assert up_updates(W, h) == sum(W - 2 * h * t for t in range(1, L))
+            assert down_updates(W, h) == sum(2 * h * t for t in range(1, L + 1))
+
+
+# ---- plain-Python model of the swept rule on the staircase rows ---------------------------------------------------
+class Model:
+    """Integer stencil `new[x] = sum_k c_k * prev[x+k]` (radius h); S = 2 makes even tiers accumulate onto the value two
+    tiers below (the paper's RK2 structure, Fig. 5 `+=`), odd tiers overwrite."""
+
+    def __init__(self, nx, h, S, u0):
+        self.nx, self.h, self.S = nx, h, S
+        self.R = [np.array(u0, dtype=object), np.zeros(nx, dtype=object)]
+        self.coef = {1: (1, 2, 1), 2: (1, -3, 5, 2, -1)}[h]
+        self.count = np.zeros(nx, dtype=np.int64)      # tier of the newest value held for every point (checked at the end)
+        self.updates = 0
+
+    def point(self, win, base, odd):
+        v = sum(c * x for c, x in zip(self.coef, win))
+        if self.S == 2 and not odd:
+            return base + 3 * v
+        return v
+
+    def naive(self, nsteps):
+        a = self.R[0].copy()
+        nx, h = self.nx, self.h
+        for _ in range(nsteps):
+            if self.S == 1:
+                a = np.array([self.point([a[(i + k) % nx] for k in range(-h, h + 1)], None, True) for i in range(nx)], dtype=object)
+            else:
+                p = np.array([self.point([a[(i + k) % nx] for k in range(-h, h + 1)], None, True) for i in range(nx)], dtype=object)
+                a = np.array([self.point([p[(i + k) % nx] for k in range(-h, h + 1)], a[i], False) for i in range(nx)], dtype=object)
+        return a
+
+    def tile(self, mode, W, g0):
+        nx, h = self.nx, self.h
+        L, c = W // (2 * h), W // 2
+        row = [{x: self.R[0][(g0 + x) % nx] for x in range(W)}, {}]
+        if mode != "up":
+            row[1] = {x: self.R[1][(g0 + x) % nx] for x in range(-h, W + h)}
+        spans = []
+        if mode != "up":
+            spans += [(t, c - h * t, c + h * t) for t in range(1, L + 1)]
+        if mode != "down":
+            spans += [(t, h * t, W - h * t) for t in range(1, L)]
+        for t, lo, hi in spans:
+            src, dst = row[(t - 1) & 1], row[t & 1]
+            new = {x: self.point([src[x + k] for k in range(-h, h + 1)], row[0].get(x), bool(t & 1)) for x in range(lo, hi)}
+            dst.update(new)
+            self.updates += hi - lo
+        return row
+
+    def launch(self, mode, W, offset):
+        nx, h = self.nx, self.h
+        rows = [self.tile(mode, W, t * W + offset) for t in range(nx // W)]     # all tiles read before any writes ...
+        for t, row in enumerate(rows):                                           # ... (snapshot semantics; A4 shows in-place is equal)
+            g0 = t * W + offset
+            for x in range(W):
+                self.R[0][(g0 + x) % nx] = row[0][x]
+            if mode != "down":
+                for x in range(h, W - h):
+                    self.R[1][(g0 + x) % nx] = row[1][x]
+
+    def classic(self, nsteps):
+        self.R[0] = self.naive(nsteps)
+        self.updates += nsteps * self.S * self.nx
+
+    def run_plan(self, plan):
+        for kind, W, offset, count in plan:
+            if kind == sw.LAUNCH_CLASSIC:
+                self.classic(count)
+            elif kind == sw.LAUNCH_UP:
+                self.launch("up", W, offset)
+            elif kind == sw.LAUNCH_DOWN:
+                self.launch("down", W, offset)
+            elif kind == sw.LAUNCH_DIAMOND:
+                for k in range(count):
+                    self.launch("diamond", W, offset if k % 2 == 0 else (0 if offset else W // 2))
+            elif kind == sw.LAUNCH_CHAIN:
+                for p in range(count + 1):
+                    self.launch("up" if p == 0 else ("down" if p == count else "diamond"), W, W // 2 if p & 1 else 0)
+            else:
+                raise AssertionError(kind)
+
+
+CASES = [
+    # problem, nx, W, nsteps
+    (sw.HEAT, 64, 16, 8 * 3),            # 3 half-cycles, no remainder: closes on the shifted alignment
+    (sw.HEAT, 64, 16, 8 * 4 + 7),        # remainder 7 = 4 + 2 + 1 classic
+    (sw.HEAT, 32, 32, 16 * 2 + 5),       # single tile wrapping onto itself
+    (sw.HEAT, 64, 8, 3),                 # fewer steps than one half-cycle: q = 0
+    (sw.KS, 64, 16, 2 * 3 + 1),          # h = 2, S = 2: 2 timesteps per half-cycle of 16 points
+    (sw.KS, 64, 32, 4 * 2 + 3),
+    (sw.EULER, 32, 8, 5),
+]
+
+
+@pytest.mark.parametrize("chain", [False, True], ids=["per-launch", "chain"])
+@pytest.mark.parametrize("problem,nx,W,nsteps", CASES)
+def test_plan_executed_on_the_model_equals_naive_stepping(problem, nx, W, nsteps, chain):
+    h, S = sw.RADIUS[problem], sw.STAGES[problem]
+    rng = np.random.default_rng(1612)
+    u0 = [int(v) for v in rng.integers(-5, 6, nx)]
+    plan = sw.plan(problem, nx, nsteps, W, kernel=sw.KERNEL_SMEM, chain=chain)
+    m = Model(nx, h, S, u0)
+    m.run_plan(plan)
+    ref = Model(nx, h, S, u0).naive(nsteps)
+    assert list(m.R[0]) == list(ref)
+    # every (point, tier) exactly once: the update count is nx * S * nsteps, whatever the decomposition
+    assert m.updates == nx * S * nsteps
+
+
+def test_plan_structure_and_launch_counts():
+    # config 1: 10 000 = 312 * 32 + 16
+    plan = sw.plan(sw.HEAT, 1024, 10000, 64, kernel=sw.KERNEL_SMEM, chain=False)
+    assert plan == [(sw.LAUNCH_UP, 32, 0, 1), (sw.LAUNCH_DOWN, 32, 16, 1), (sw.LAUNCH_UP, 64, 0, 1), (sw.LAUNCH_DIAMOND, 64, 32, 311),
+                    (sw.LAUNCH_DOWN, 64, 0, 1)]
+    # the WAVE kernels offer W >= 64 for heat: the 16 remainder steps run on the classic kernel, the sweep is one chained launch
+    plan = sw.plan(sw.HEAT, 1024, 10000, 64, kernel=sw.KERNEL_WAVE, chain=True)
+    assert plan == [(sw.LAUNCH_CLASSIC, 0, 0, 16), (sw.LAUNCH_CHAIN, 64, 0, 312)]
+    # config 2 remainders: 50 000 steps, W = 1024: r = 336 = 256 + 64 + 16
+    plan = sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE, chain=True)
+    assert [(k, W) for k, W, _, _ in plan] == [(sw.LAUNCH_UP, 512), (sw.LAUNCH_DOWN, 512), (sw.LAUNCH_UP, 128), (sw.LAUNCH_DOWN, 128),
+                                               (sw.LAUNCH_CLASSIC, 0), (sw.LAUNCH_CHAIN, 1024)]
+    assert plan[-1][3] == 97 and plan[-2][3] == 16
+    # q = 0: everything classic or narrower tiles
+    assert sw.plan(sw.KS, 4096, 3, 128, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_CLASSIC, 0, 0, 3)]
+    assert sw.plan(sw.KS, 4096, 0, 128) == []
+
+
+def test_plan_rejects_illegal_widths():
+    for bad in (0, 3, 48, 4, 1 << 13):
+        with pytest.raises(sw.SweptError):
+            sw.plan(sw.KS, 4096, 100, bad, kernel=sw.KERNEL_SMEM)
+    with pytest.raises(sw.SweptError):
+        sw.plan(sw.HEAT, 4096, 100, 32, kernel=sw.KERNEL_WAVE)      # WAVE heat starts at W = 64
+    with pytest.raises(sw.SweptError):
+        sw.plan(sw.HEAT, 1000, 100, 64)

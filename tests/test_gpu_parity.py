@@ -10,14 +10,14 @@ import pytest
 
 import paper_1612_02495_b200 as sw
 import workloads as wl
-from gpu_util import (TOL, assert_bits_equal, rel_max, run_naive, run_oracle, run_swept, solver_for, to_dev, width_ok)
+from gpu_util import (VARIANTS, VARIANT_IDS, TOL, assert_bits_equal, rel_max, run_naive, run_oracle, run_swept, solver_for, to_dev, width_ok)
 
 pytestmark = pytest.mark.gpu
 
 PROBLEMS = [wl.HEAT, wl.KS, wl.EULER]
 DTYPES = [np.float64, np.float32]
-KERNELS = [sw.KERNEL_SMEM, sw.KERNEL_WAVE]
-KNAME = {sw.KERNEL_SMEM: "smem", sw.KERNEL_WAVE: "wave"}
+KERNELS = VARIANTS            # (kernel family, chain): smem, wave (one launch per half-cycle), chain (launch-free sweep)
+KNAME = dict(zip(VARIANTS, VARIANT_IDS))
 
 
 def _noise(problem, nx):
@@ -54,7 +54,7 @@ def _sph(problem, W):
     return wl.steps_per_half_cycle(problem, W)
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 @pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
 @pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
 @pytest.mark.parametrize("W", [8, 32, 64, 128, 256, 512, 1024, 2048])
@@ -72,7 +72,7 @@ def test_swept_matches_naive_bitwise(problem, dtype, W, kernel):
     assert_bits_equal(got, ref, f"swept({KNAME[kernel]}) vs naive W={W}")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 @pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
 @pytest.mark.parametrize("q", [1, 2, 4, 5])
 def test_swept_half_cycle_counts(problem, q, kernel):
@@ -85,7 +85,7 @@ def test_swept_half_cycle_counts(problem, q, kernel):
     assert_bits_equal(run_swept(w, np.float64, nsteps, W, kernel), run_naive(w, np.float64, nsteps), f"q={q}")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 @pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
 def test_swept_single_tile_wraps_onto_itself(problem, kernel):
     W = nx = 256
@@ -96,7 +96,7 @@ def test_swept_single_tile_wraps_onto_itself(problem, kernel):
     assert_bits_equal(run_swept(w, np.float64, nsteps, W, kernel), run_naive(w, np.float64, nsteps), "nx == W")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 @pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
 def test_swept_translation_equivariance_bitwise(problem, kernel):
     """A circular shift by a non-multiple of W commutes with the swept run bit for bit (exposes tile-edge bugs)."""
@@ -111,7 +111,7 @@ def test_swept_translation_equivariance_bitwise(problem, kernel):
     assert_bits_equal(b.reshape(u0.shape), np.roll(a.reshape(u0.shape), shift, axis=1), "shift equivariance")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 def test_result_independent_of_tile_width(kernel):
     w = _noise(wl.KS, 4096)
     outs = []
@@ -124,7 +124,7 @@ def test_result_independent_of_tile_width(kernel):
         assert_bits_equal(o, outs[0], "tile-width independence")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 def test_swept_graph_replay_matches_plain(kernel):
     w = _noise(wl.HEAT, 4096)
     if not width_ok(w, np.float64, 128, kernel):
@@ -136,7 +136,7 @@ def test_swept_graph_replay_matches_plain(kernel):
 # ------------------------------------------------------------------------------------------------------------
 # swept vs oracle on the configs (BASELINE.json)
 # ------------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 def test_config1_heat_full_run_matches_oracle(kernel):
     """Config 1 exactly: heat fp64, nx=1024, r=0.25, 10 000 steps, W=64 (312 half-cycles + 16 remainder steps)."""
     w = wl.heat_config1()
@@ -148,7 +148,7 @@ def test_config1_heat_full_run_matches_oracle(kernel):
     assert_bits_equal(got, ref, "config 1")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 @pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
 @pytest.mark.parametrize("problem,nx,nsteps,W", [(wl.HEAT, 1 << 14, 3000, 256), (wl.KS, 1 << 14, 2000, 256), (wl.EULER, 1 << 12, 1500, 128)],
                          ids=["heat-c2", "ks-c3", "euler-c4"])
@@ -200,12 +200,13 @@ def test_run_host_round_trip_and_info():
         assert_bits_equal(h.numpy(), run_naive(w, np.float64, 40), "run_host")
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["smem", "wave"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=VARIANT_IDS)
 def test_tuner_returns_a_legal_width_and_default_run_uses_it(kernel):
     import torch
     w = _noise(wl.HEAT, 1 << 14)
     with solver_for(w, np.float32, max_tile_width=512) as s:
-        s.set_option(sw.OPT_KERNEL, kernel)
+        s.set_option(sw.OPT_KERNEL, kernel[0])
+        s.set_option(sw.OPT_CHAIN, kernel[1])
         if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512)):
             pytest.skip("kernel offers no width")
         scratch = to_dev(w.initial(np.float32))
@@ -222,3 +223,65 @@ def test_alu_peak_microbenchmark_is_plausible():
     p64 = sw.measure_alu_peak(sw.F64)["instr_per_s"]
     p32 = sw.measure_alu_peak(sw.F32)["instr_per_s"]
     assert 1e12 < p64 < 1e14 and 1e12 < p32 < 2e14
+
+
+# ------------------------------------------------------------------------------------------------------------
+# launch-free sweep (SWEPT_OPT_CHAIN): flag-ordered persistent kernel
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+@pytest.mark.parametrize("nx,W,q", [(128, 128, 9), (256, 128, 12), (1 << 12, 128, 40), (1 << 20, 128, 5), (1 << 16, 512, 7)])
+def test_chain_many_phases_few_and_many_tiles(problem, nx, W, q):
+    """One tile wrapping onto itself, two tiles (each the other's both neighbours), fewer tiles than SMs, and far more
+    tiles than resident warps (8192 tiles: items of several phases in flight at once): the chained launch equals the
+    classic path bit for bit."""
+    from gpu_util import CHAIN
+    w = _noise(problem, nx)
+    if not width_ok(w, np.float64, W, CHAIN):
+        pytest.skip("width not offered")
+    nsteps = q * _sph(problem, W)
+    assert_bits_equal(run_swept(w, np.float64, nsteps, W, CHAIN), run_naive(w, np.float64, nsteps), f"chain nx={nx} W={W} q={q}")
+
+
+@pytest.mark.parametrize("wpb", [1, 2, 4, 8])
+@pytest.mark.parametrize("cap", [0, 1, 3])
+def test_chain_launch_shapes(wpb, cap):
+    from gpu_util import CHAIN
+    w = _noise(wl.KS, 1 << 15)
+    nsteps = 11 * _sph(wl.KS, 256) + 5
+    got = run_swept(w, np.float32, nsteps, 256, CHAIN, opts={sw.OPT_WARPS_PER_BLOCK: wpb, sw.OPT_BLOCKS_PER_SM: cap})
+    assert_bits_equal(got, run_naive(w, np.float32, nsteps), f"chain wpb={wpb} cap={cap}")
+
+
+def test_chain_repeated_calls_reuse_the_flags_and_plan_matches_launch_count():
+    import torch
+    w = _noise(wl.HEAT, 1 << 13)
+    with solver_for(w, np.float64) as s:
+        u = to_dev(w.initial(np.float64))
+        total = 0
+        for nsteps in (64 * 3, 64 * 8 + 17, 5, 64):
+            s.swept_run(u, nsteps, 128)
+            total += nsteps
+            kinds = [k for k, *_ in sw.plan(wl.HEAT, w.nx, nsteps, 128)]
+            assert s.info()["launches_last_call"] == sum(
+                c if k in (sw.LAUNCH_CLASSIC, sw.LAUNCH_DIAMOND) else 1 for k, _, _, c in sw.plan(wl.HEAT, w.nx, nsteps, 128)), kinds
+        torch.cuda.synchronize()
+        assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float64, total), "four chained calls back to back")
+
+
+def test_chain_graph_replay_and_two_streams():
+    """Two solvers on two streams run chained sweeps concurrently (each handle owns its flags)."""
+    import torch
+    w = _noise(wl.HEAT, 1 << 14)
+    s1, s2 = solver_for(w, np.float64), solver_for(w, np.float64)
+    s2.set_option(sw.OPT_SWEPT_GRAPH, 1)
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    u1, u2 = to_dev(w.initial(np.float64)), to_dev(w.initial(np.float64))
+    torch.cuda.synchronize()
+    for _ in range(3):
+        s1.swept_run(u1, 1000, 256, stream=st1)
+        s2.swept_run(u2, 1000, 256, stream=st2)
+    torch.cuda.synchronize()
+    ref = run_naive(w, np.float64, 3000)
+    assert_bits_equal(u1.cpu().numpy(), ref, "stream 1")
+    assert_bits_equal(u2.cpu().numpy(), ref, "stream 2 (graph replay)")
+    s1.close(); s2.close()
