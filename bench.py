@@ -40,7 +40,7 @@ FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP instructions of one point updat
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--problem", default="heat", choices=["heat", "ks", "euler"])
@@ -50,6 +50,8 @@ def parse():
     ap.add_argument("--tile-width", type=int, default=0, help="0 = tuned (swept_tune)")
     ap.add_argument("--kernel", default="wave", choices=["wave", "smem"])
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--variants", default="", help="--sweep: comma list of chain,wave,smem (default all)")
+    ap.add_argument("--no-chain", action="store_true", help="one launch per half-cycle (PAPER.md:98) instead of the launch-free sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
     return ap.parse_args()
@@ -201,19 +203,24 @@ def run_sweep(args):
             s.set_option(sw.OPT_NAIVE_GRAPH, 1)
             t = timed(lambda: s.naive_run(u, ns_naive))
             row["naive_graph"] = nx * ns_naive / t / 1e9
-            for kname, kid in (("wave", sw.KERNEL_WAVE), ("smem", sw.KERNEL_SMEM)):
+            # chain = launch-free sweep (one persistent launch); wave / smem = one launch per half-cycle, plain or CUDA graph
+            for kname, kid, chain, graphs in (("chain", sw.KERNEL_WAVE, 1, (0,)), ("wave", sw.KERNEL_WAVE, 0, (0, 1)), ("smem", sw.KERNEL_SMEM, 0, (0, 1))):
+                if args.variants and kname not in args.variants.split(","):
+                    continue
                 s.set_option(sw.OPT_KERNEL, kid)
+                s.set_option(sw.OPT_CHAIN, chain)
                 for W in (32, 64, 128, 256, 512, 1024, 2048):
                     if W > nx or not s.tile_width_ok(W):
                         continue
-                    for graph in (0, 1):
+                    for graph in graphs:
                         s.set_option(sw.OPT_SWEPT_GRAPH, graph)
                         u.copy_(u0)
                         t = timed(lambda: s.swept_run(u, w.nsteps, W), reps=3 if nx <= (1 << 20) else 2)
                         row["swept"][f"{kname}/W={W}/{'graph' if graph else 'plain'}"] = nx * w.nsteps / t / 1e9
         best = max(row["swept"], key=row["swept"].get)
         row["best"], row["best_value"] = best, row["swept"][best]
-        best_paper = max((k for k in row["swept"] if k.startswith("smem") and k.endswith("plain")), key=row["swept"].get)
+        paper = [k for k in row["swept"] if k.startswith("smem") and k.endswith("plain")]
+        best_paper = max(paper, key=row["swept"].get) if paper else best
         row["best_paper_style"], row["best_paper_style_value"] = best_paper, row["swept"][best_paper]
         row["speedup_vs_naive"] = row["best_value"] / row["naive"]
         row["speedup_vs_naive_graph"] = row["best_value"] / row["naive_graph"]
@@ -260,6 +267,7 @@ def main():
     kernel = sw.KERNEL_WAVE if args.kernel == "wave" else sw.KERNEL_SMEM
     s = sw.Solver(w.problem, w.nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma)
     s.set_option(sw.OPT_KERNEL, kernel)
+    s.set_option(sw.OPT_CHAIN, 0 if args.no_chain else 1)
     if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512, 1024)):
         kernel = sw.KERNEL_SMEM
         s.set_option(sw.OPT_KERNEL, kernel)
@@ -328,29 +336,44 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the diamond): average launch duration by differencing two runs ----
-    def half_cycles(q):
-        return lambda: s.swept_run(u, q * sph, W)
-
-    qa, qb = 16, 48
-    for q in (qa, qb):
-        half_cycles(q)()
-    ta = min(timed(half_cycles(qa), 1) for _ in range(3))
-    tb = min(timed(half_cycles(qb), 1) for _ in range(3))
-    t_diamond = (tb - ta) / (qb - qa)
+    # ---- roofline of the dominant kernel -------------------------------------------------------------------
+    # chain (default): ONE launch of swept_chain_kernel runs the step's q half-cycles = nx*L*q stage-updates; it is timed
+    # alone (nsteps = q*sph has no remainder, so the plan is that single launch + the memset of its flags).
+    # per-launch kernels (--no-chain / smem): the diamond launch, by differencing two runs of qa and qb half-cycles.
     H, S = sw.RADIUS[w.problem], sw.STAGES[w.problem]
     L = W // (2 * H)
-    stage_updates = w.nx * L                                   # per diamond launch: every point advances L tiers
+    chain = kernel == sw.KERNEL_WAVE and not args.no_chain
+    if chain:
+        q = max(1, w.nsteps // sph)
+        assert [k for k, *_ in sw.plan(w.problem, w.nx, q * sph, W, dtype=sw_dtype)] == [sw.LAUNCH_CHAIN]
+        run_q = lambda: s.swept_run(u, q * sph, W)
+        run_q()
+        t_launch = min(timed(run_q, 1) for _ in range(3))
+        stage_updates = w.nx * L * q
+        kname = f"swept_chain_kernel W={W} ({q} half-cycles in one launch)"
+    else:
+        def half_cycles(n):
+            return lambda: s.swept_run(u, n * sph, W)
+        qa, qb = 16, 48
+        for n in (qa, qb):
+            half_cycles(n)()
+        ta = min(timed(half_cycles(qa), 1) for _ in range(3))
+        tb = min(timed(half_cycles(qb), 1) for _ in range(3))
+        t_launch = (tb - ta) / (qb - qa)
+        stage_updates = w.nx * L                               # per diamond launch: every point advances L tiers
+        kname = f"swept diamond ({'wave' if kernel == sw.KERNEL_WAVE else 'smem'}) W={W}"
     fpi = FP_INSTR_PER_STAGE_UPDATE[(args.problem, args.dtype)]
     peak = sw.measure_alu_peak(sw_dtype)["instr_per_s"]
-    achieved = fpi * stage_updates / t_diamond if fpi else None
+    nominal = 148 * (64 if args.dtype == "f64" else 128) * 1.965e9
+    achieved = fpi * stage_updates / t_launch if fpi else None
     roofline = {
-        "bound": "alu", "kernel": f"swept diamond ({'wave' if kernel == sw.KERNEL_WAVE else 'smem'}) W={W}",
+        "bound": "alu", "kernel": kname,
         "achieved": achieved / 1e12 if achieved else None, "peak": peak / 1e12, "unit": "T FP-instr/s (thread-level)",
         "frac": (achieved / peak) if achieved else None, "traffic": None,
         "peak_source": "measured FMA-chain microbenchmark (swept_measure_alu_peak), same process",
-        "launch_ms": t_diamond * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
-        "hbm_algorithmic_bytes_per_launch": int(4 * w.nx * sw.NCOMP[w.problem] * u.element_size()),
+        "peak_nominal": nominal / 1e12, "frac_nominal": (achieved / nominal) if achieved else None,
+        "launch_ms": t_launch * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
+        "hbm_algorithmic_bytes_per_launch": int(4 * w.nx * sw.NCOMP[w.problem] * u.element_size() * (q if chain else 1)),
     }
 
     # ---- classic path on the same workload (context: swept / classic speedup) ------------------------------
@@ -391,7 +414,7 @@ def main():
         "config": {
             "workload": f"BASELINE.json configs[1]: {w.name}, FTCS periodic r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
                         f"{w.nsteps} timesteps per step" if args.problem == "heat" else f"{w.name} nx={w.nx} {w.nsteps} timesteps per step",
-            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": args.kernel if kernel == sw.KERNEL_WAVE else "smem",
+            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": ("chain" if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
         },

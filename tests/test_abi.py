@@ -14,7 +14,7 @@ HEADER = os.path.join(ROOT, "include", "swept1d.h")
 def _declared_functions():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"^\s*(?:const\s+char\s*\*|int)\s*\**\s*(\w+)\s*\(", src, flags=re.M)
+    names = re.findall(r"^\s*(?:const\s+char\s*\*|int64_t|int)\s*\**\s*(\w+)\s*\(", src, flags=re.M)
     return sorted(set(names))
 
 
