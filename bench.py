@@ -21,7 +21,6 @@ import os
 import statistics
 import subprocess
 import sys
-import threading
 import time
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
@@ -35,6 +34,17 @@ import workloads as wl  # noqa: E402
 FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP instructions of one point update
     ("heat", "f64"): 3, ("heat", "f32"): 3, ("ks", "f64"): 11, ("ks", "f32"): 11, ("euler", "f64"): 0, ("euler", "f32"): 0,
 }
+
+
+def traffic_of(args, w, W, chain):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel's launch, from the committed `ncu --set full`
+    capture of this very configuration (profiles/traffic.json names the report it was read from); None if there is none."""
+    try:
+        tab = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        key = f"{args.problem}_{args.dtype}_nx{w.nx}_W{W}_{'chain' if chain else args.kernel}_nsteps{w.nsteps}"
+        return tab.get(key, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
 
 
 def parse():
@@ -68,31 +78,37 @@ def workload(args) -> wl.Workload:
 # clocks: sample nvidia-smi during the timed region (B200_PROFILING.md "clocks line")
 # ---------------------------------------------------------------------------------------------------------------
 class ClockSampler:
+    """ONE long-lived `nvidia-smi -lms` process started before the timed region and read after it: no fork, no Python
+    thread and no GIL traffic while the steps are being timed."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index: int):
-        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
-
-    def _run(self):
-        while not self._stop.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
-                                     capture_output=True, text=True, timeout=5).stdout.strip()
-                if out:
-                    self.rows.append([c.strip() for c in out.split(",")])
-            except Exception:
-                pass
-            self._stop.wait(0.05)
+    def __init__(self, index: int, period_ms: int = 20):
+        self.index, self.period_ms, self.rows, self._p = index, period_ms, [], None
 
     def __enter__(self):
-        self._t = threading.Thread(target=self._run, daemon=True)
-        self._t.start()
+        try:
+            self._p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index),
+                                        "-lms", str(self.period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            time.sleep(0.3)          # let it attach and print its first rows before the timed region starts
+        except Exception:
+            self._p = None
         return self
 
     def __exit__(self, *exc):
-        self._stop.set()
-        self._t.join(timeout=6)
+        if self._p is None:
+            return
+        time.sleep(0.05)
+        self._p.terminate()
+        try:
+            out, _ = self._p.communicate(timeout=5)
+        except Exception:
+            self._p.kill()
+            out = ""
+        for line in out.splitlines():
+            cols = [c.strip() for c in line.split(",")]
+            if len(cols) >= 7:
+                self.rows.append(cols)
 
     def summary(self) -> dict:
         sm, mx, reasons = [], [], set()
@@ -369,7 +385,7 @@ def main():
     roofline = {
         "bound": "alu", "kernel": kname,
         "achieved": achieved / 1e12 if achieved else None, "peak": peak / 1e12, "unit": "T FP-instr/s (thread-level)",
-        "frac": (achieved / peak) if achieved else None, "traffic": None,
+        "frac": (achieved / peak) if achieved else None, "traffic": traffic_of(args, w, W, chain),
         "peak_source": "measured FMA-chain microbenchmark (swept_measure_alu_peak), same process",
         "peak_nominal": nominal / 1e12, "frac_nominal": (achieved / nominal) if achieved else None,
         "launch_ms": t_launch * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
