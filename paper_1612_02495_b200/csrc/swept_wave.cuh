@@ -113,6 +113,25 @@ __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real 
                 const int t = tb + n;
                 const bool odd = (t & 1) != 0;
                 const bool pact = (MODE == MODE_DIAMOND) ? true : (MODE == MODE_UP ? (t > L) : (t <= L));
+                if constexpr (P::GROUPED) {
+                    // the D points of this n lie on one tier at neighbouring x and read X[k][D n .. D n + 2D) only, none of
+                    // which another of them writes before reading: one call that shares work between them
+                    T win[NC][2 * D], out[D][NC];
+#pragma unroll
+                    for (int k = 0; k < NC; ++k)
+#pragma unroll
+                        for (int m = 0; m < 2 * D; ++m) win[k][m] = X[k][D * n + m];
+                    P::group_sel(c, odd, win, old, out);
+#pragma unroll
+                    for (int rho = 0; rho < D; ++rho) {
+                        const int q = (D - 1 - rho) + D * n;
+#pragma unroll
+                        for (int k = 0; k < NC; ++k) {
+                            old[rho][k] = X[k][q + D];
+                            X[k][q + D] = pact ? out[rho][k] : X[k][q + D];
+                        }
+                    }
+                } else {
 #pragma unroll
                 for (int rho = 0; rho < D; ++rho) {
                     const int q = (D - 1 - rho) + D * n;   // row residue r = D-1-rho; window X[k][q .. q+D], target X[k][q+D]
@@ -127,6 +146,7 @@ __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real 
                         old[rho][k] = X[k][q + D];
                         X[k][q + D] = pact ? out[k] : X[k][q + D];
                     }
+                }
                 }
             }
             if (MODE != MODE_DOWN && lane == 31) {    // the row outputs: newest value of row rho is column PW-D+r
