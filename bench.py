@@ -31,8 +31,12 @@ import numpy as np  # noqa: E402
 
 import workloads as wl  # noqa: E402
 
-FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP instructions of one point update
-    ("heat", "f64"): 3, ("heat", "f32"): 3, ("ks", "f64"): 11, ("ks", "f32"): 11, ("euler", "f64"): 0, ("euler", "f32"): 0,
+FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP-pipe instructions of one point update (DESIGN.md section 5.3 / 5.6)
+    ("heat", "f64"): 3, ("heat", "f32"): 3, ("ks", "f64"): 11, ("ks", "f32"): 11,
+    # Euler: SASS count of Euler<T>::group_sel (4 cells: 7 differences, 6 limited slopes, 5 face fluxes with IEEE
+    # division and square root expanded inline) / 4: f64 (109 DADD + 199 DFMA + 145 DMUL + 44 DSETP) / 4,
+    # f32 (122 FADD + 129 FFMA + 131 FMUL + 40 FSETP + 5 FMNMX) / 4
+    ("euler", "f64"): 124.25, ("euler", "f32"): 106.75,
 }
 
 
@@ -72,6 +76,25 @@ def workload(args) -> wl.Workload:
     if args.nsteps:
         w.nsteps = args.nsteps
     return w
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# ranks: "replicas only" -- every rank times its own replica; the job's time is the slowest rank's
+# ---------------------------------------------------------------------------------------------------------------
+def max_over_ranks(seconds: float, world: int, device="cpu") -> float:
+    """MAX over ranks of a locally measured duration (the contract's max-over-ranks timing); no collective on the data path."""
+    if world <= 1:
+        return float(seconds)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(nx: int, nsteps: int, steps: int, world: int, t_max: float) -> float:
+    """Whole-job GPts*steps/s: the units ALL ranks processed (world independent replicas) / the slowest rank's time."""
+    return world * nx * nsteps * steps / t_max / 1e9
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -326,11 +349,8 @@ def main():
         t_dev = timed(step_dev, args.steps)
         barrier()
     launches = s.info()["launches_total"] - l0
-    t = torch.tensor([t_dev], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    t_dev_max = float(t.item())
-    value = world * w.nx * w.nsteps * args.steps / t_dev_max / 1e9
+    t_dev_max = max_over_ranks(t_dev, world, "cuda")
+    value = job_value(w.nx, w.nsteps, args.steps, world, t_dev_max)
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----------------
     h_buf = u0_host.clone().pin_memory()
@@ -341,10 +361,7 @@ def main():
     step_e2e()
     barrier()
     t_e2e = timed(step_e2e, args.steps)
-    t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * w.nx * w.nsteps * args.steps / float(t.item()) / 1e9
+    e2e_value = job_value(w.nx, w.nsteps, args.steps, world, max_over_ranks(t_e2e, world, "cuda"))
     field_bytes = int(u.numel() * u.element_size())
 
     if rank != 0:
