@@ -45,7 +45,7 @@ def traffic_of(args, w, W, chain):
     capture of this very configuration (profiles/traffic.json names the report it was read from); None if there is none."""
     try:
         tab = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        key = f"{args.problem}_{args.dtype}_nx{w.nx}_W{W}_{'chain' if chain else args.kernel}_nsteps{w.nsteps}"
+        key = f"{args.problem}_{args.dtype}_nx{w.nx}_W{W}_{chain if chain else args.kernel}_nsteps{w.nsteps}"
         return tab.get(key, {}).get("dram_bytes_per_launch")
     except Exception:
         return None
@@ -64,8 +64,10 @@ def parse():
     ap.add_argument("--tile-width", type=int, default=0, help="0 = tuned (swept_tune)")
     ap.add_argument("--kernel", default="wave", choices=["wave", "smem"])
     ap.add_argument("--sweep", action="store_true")
-    ap.add_argument("--variants", default="", help="--sweep: comma list of chain,wave,smem (default all)")
-    ap.add_argument("--no-chain", action="store_true", help="one launch per half-cycle (PAPER.md:98) instead of the launch-free sweep")
+    ap.add_argument("--variants", default="", help="--sweep: comma list of band,chain,wave,smem (default all)")
+    ap.add_argument("--chain", type=int, default=2, choices=[0, 1, 2],
+                    help="launch-free sweep: 2 = streaming bands (default), 1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
+    ap.add_argument("--no-chain", action="store_true", help="same as --chain 0")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
     return ap.parse_args()
@@ -243,7 +245,8 @@ def run_sweep(args):
             t = timed(lambda: s.naive_run(u, ns_naive))
             row["naive_graph"] = nx * ns_naive / t / 1e9
             # chain = launch-free sweep (one persistent launch); wave / smem = one launch per half-cycle, plain or CUDA graph
-            for kname, kid, chain, graphs in (("chain", sw.KERNEL_WAVE, 1, (0,)), ("wave", sw.KERNEL_WAVE, 0, (0, 1)), ("smem", sw.KERNEL_SMEM, 0, (0, 1))):
+            for kname, kid, chain, graphs in (("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0,)), ("wave", sw.KERNEL_WAVE, 0, (0, 1)),
+                                              ("smem", sw.KERNEL_SMEM, 0, (0, 1))):
                 if args.variants and kname not in args.variants.split(","):
                     continue
                 s.set_option(sw.OPT_KERNEL, kid)
@@ -306,7 +309,8 @@ def main():
     kernel = sw.KERNEL_WAVE if args.kernel == "wave" else sw.KERNEL_SMEM
     s = sw.Solver(w.problem, w.nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma)
     s.set_option(sw.OPT_KERNEL, kernel)
-    s.set_option(sw.OPT_CHAIN, 0 if args.no_chain else 1)
+    chain_opt = 0 if args.no_chain else args.chain
+    s.set_option(sw.OPT_CHAIN, chain_opt)
     if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512, 1024)):
         kernel = sw.KERNEL_SMEM
         s.set_option(sw.OPT_KERNEL, kernel)
@@ -375,15 +379,16 @@ def main():
     # per-launch kernels (--no-chain / smem): the diamond launch, by differencing two runs of qa and qb half-cycles.
     H, S = sw.RADIUS[w.problem], sw.STAGES[w.problem]
     L = W // (2 * H)
-    chain = kernel == sw.KERNEL_WAVE and not args.no_chain
+    chain = kernel == sw.KERNEL_WAVE and chain_opt != 0
     if chain:
         q = max(1, w.nsteps // sph)
-        assert [k for k, *_ in sw.plan(w.problem, w.nx, q * sph, W, dtype=sw_dtype)] == [sw.LAUNCH_CHAIN]
+        assert [k for k, *_ in sw.plan(w.problem, w.nx, q * sph, W, dtype=sw_dtype, chain=chain_opt)] == [sw.LAUNCH_BAND if chain_opt == 2 else sw.LAUNCH_CHAIN]
         run_q = lambda: s.swept_run(u, q * sph, W)
         run_q()
         t_launch = min(timed(run_q, 1) for _ in range(3))
         stage_updates = w.nx * L * q
-        kname = f"swept_chain_kernel W={W} ({q} half-cycles in one launch)"
+        band = s.info()["last_sweep_launch"] == sw.LAUNCH_BAND      # False: the band schedule did not fit, swept_chain_kernel ran
+        kname = f"{'swept_band_kernel' if band else 'swept_chain_kernel'} W={W} ({q} half-cycles in one launch)"
     else:
         def half_cycles(n):
             return lambda: s.swept_run(u, n * sph, W)
@@ -394,6 +399,7 @@ def main():
         tb = min(timed(half_cycles(qb), 1) for _ in range(3))
         t_launch = (tb - ta) / (qb - qa)
         stage_updates = w.nx * L                               # per diamond launch: every point advances L tiers
+        band = False
         kname = f"swept diamond ({'wave' if kernel == sw.KERNEL_WAVE else 'smem'}) W={W}"
     fpi = FP_INSTR_PER_STAGE_UPDATE[(args.problem, args.dtype)]
     peak = sw.measure_alu_peak(sw_dtype)["instr_per_s"]
@@ -402,11 +408,13 @@ def main():
     roofline = {
         "bound": "alu", "kernel": kname,
         "achieved": achieved / 1e12 if achieved else None, "peak": peak / 1e12, "unit": "T FP-instr/s (thread-level)",
-        "frac": (achieved / peak) if achieved else None, "traffic": traffic_of(args, w, W, chain),
+        "frac": (achieved / peak) if achieved else None, "traffic": traffic_of(args, w, W, (("band" if band else "chain") if chain else "")),
         "peak_source": "measured FMA-chain microbenchmark (swept_measure_alu_peak), same process",
         "peak_nominal": nominal / 1e12, "frac_nominal": (achieved / nominal) if achieved else None,
         "launch_ms": t_launch * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
-        "hbm_algorithmic_bytes_per_launch": int(4 * w.nx * sw.NCOMP[w.problem] * u.element_size() * (q if chain else 1)),
+        # staircase bytes: per half-cycle every tile reads and writes both edges (4 W values), the band kernel only the
+        # upper-right edge (2 W values: lane 31's row outputs out, lane 0's row feed in)
+        "hbm_algorithmic_bytes_per_launch": int((2 if band else 4) * w.nx * sw.NCOMP[w.problem] * u.element_size() * (q if chain else 1)),
     }
 
     # ---- classic path on the same workload (context: swept / classic speedup) ------------------------------
@@ -447,7 +455,7 @@ def main():
         "config": {
             "workload": f"BASELINE.json configs[1]: {w.name}, FTCS periodic r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
                         f"{w.nsteps} timesteps per step" if args.problem == "heat" else f"{w.name} nx={w.nx} {w.nsteps} timesteps per step",
-            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": ("chain" if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
+            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": (("band" if band else "chain") if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
         },

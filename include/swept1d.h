@@ -58,10 +58,15 @@ enum {
     SWEPT_OPT_BLOCKS_PER_SM = 2,  /* cap on resident blocks per SM for the swept kernels, 0 = none */
     SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
     SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
-    SWEPT_OPT_CHAIN = 5           /* WAVE kernels: 1 (default) = launch-free sweep, ONE persistent launch runs all
-                                     half-cycles of a swept_run, tiles ordered by per-tile flags in global memory
-                                     (beyond the paper; removes PAPER.md:232's launch/wave costs); 0 = one launch
-                                     per half-cycle as in the paper                   */
+    SWEPT_OPT_CHAIN = 5           /* WAVE kernels, launch-free sweep (beyond the paper; removes PAPER.md:232's launch / wave
+                                     costs): ONE persistent launch runs all half-cycles of a swept_run.
+                                     2 (default) = streaming bands: a warp keeps its tile's columns in registers from one
+                                         half-cycle to the next (the upper-left edge of PAPER.md Fig. 2b never leaves the
+                                         SM), only the upper-right edge travels through global memory, ordered by one
+                                         progress counter per band; falls back to 1 when the schedule does not fit.
+                                     1 = tiles handed out by an atomic counter, ordered by per-tile flags, both edges
+                                         through global memory every half-cycle.
+                                     0 = one launch per half-cycle as in the paper    */
 };
 
 /* Shared memory a block may opt in to on B200 (227 KB); swept_plan, which has no device, checks SMEM-kernel tile widths
@@ -73,8 +78,10 @@ enum {
  *   UP       upright triangles, tiles at `offset`                                  (Fig. 5)
  *   DIAMOND  `count` consecutive diamond launches, the first at `offset`, then alternating 0 <-> W/2
  *   DOWN     closing inverted triangles at `offset`
- *   CHAIN    `count` half-cycles (1 UP + (count-1) DIAMOND + 1 DOWN phases, offsets 0, W/2, 0, ...) in ONE launch */
-enum { SWEPT_LAUNCH_CLASSIC = 0, SWEPT_LAUNCH_UP = 1, SWEPT_LAUNCH_DIAMOND = 2, SWEPT_LAUNCH_DOWN = 3, SWEPT_LAUNCH_CHAIN = 4 };
+ *   CHAIN    `count` half-cycles (1 UP + (count-1) DIAMOND + 1 DOWN phases, offsets 0, W/2, 0, ...) in ONE launch
+ *   BAND     the same in ONE launch of the streaming band kernel (SWEPT_OPT_CHAIN = 2; a handle whose device cannot hold
+ *            the band schedule runs the entry as CHAIN)                                                              */
+enum { SWEPT_LAUNCH_CLASSIC = 0, SWEPT_LAUNCH_UP = 1, SWEPT_LAUNCH_DIAMOND = 2, SWEPT_LAUNCH_DOWN = 3, SWEPT_LAUNCH_CHAIN = 4, SWEPT_LAUNCH_BAND = 5 };
 typedef struct {
     int kind;           /* SWEPT_LAUNCH_*                         */
     int tile_width;     /* W of the entry (0 for CLASSIC)         */
@@ -98,6 +105,8 @@ typedef struct {
     int64_t launches_total;      /* kernels enqueued through this handle since creation          */
     int sm_count;                /* multiprocessors of the device the handle lives on            */
     int max_smem_per_block;      /* opt-in shared-memory limit per block (bytes)                 */
+    int last_sweep_launch;       /* SWEPT_LAUNCH_* that ran the half-cycles of the last swept_run enqueued outside a
+                                    graph (BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet        */
 } swept_info_t;
 
 /* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's

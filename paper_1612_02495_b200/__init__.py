@@ -19,8 +19,9 @@ HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
 OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN = 0, 1, 2, 3, 4, 5
-LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN = 0, 1, 2, 3, 4
-LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain"}
+LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND = 0, 1, 2, 3, 4, 5
+LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band"}
+CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS = 0, 1, 2     # values of OPT_CHAIN (include/swept1d.h); CHAIN_BANDS is the default
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
 RADIUS = {HEAT: 1, KS: 2, EULER: 2}
@@ -52,7 +53,7 @@ class _Info(ctypes.Structure):
         ("problem", ctypes.c_int), ("dtype", ctypes.c_int), ("radius", ctypes.c_int), ("stages", ctypes.c_int), ("ncomp", ctypes.c_int),
         ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
-        ("max_smem_per_block", ctypes.c_int),
+        ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int),
     ]
 
 
@@ -215,10 +216,10 @@ def measure_alu_peak(dtype=F64, stream=None) -> dict:
     return {"instr_per_s": ips.value, "ms": ms.value}
 
 
-def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: bool = True) -> list:
+def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: int = CHAIN_BANDS) -> list:
     """The launch list `swept_run` enqueues (swept_plan; host logic, no device needed): [(kind, W, offset, count), ...]."""
     buf = (_Launch * 64)()
-    n = lib().swept_plan(int(problem), int(dtype), int(nx), int(nsteps), int(tile_width), int(kernel), int(bool(chain)), buf, 64)
+    n = lib().swept_plan(int(problem), int(dtype), int(nx), int(nsteps), int(tile_width), int(kernel), int(chain), buf, 64)
     if n < 0:
         _check(int(n))
     return [(buf[i].kind, buf[i].tile_width, buf[i].offset, buf[i].count) for i in range(min(int(n), 64))]

@@ -11,8 +11,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libswept1d.so")
-SOURCES = ["api.cu", "naive.cu", "swept_smem.cu", "swept_wave.cu", "swept_wave_heat.cu", "swept_wave_ks.cu", "swept_wave_euler.cu", "alu_peak.cu"]
-HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", os.path.join("..", "..", "include", "swept1d.h")]
+SOURCES = ["api.cu", "naive.cu", "swept_smem.cu", "swept_wave.cu", "swept_wave_heat.cu", "swept_wave_ks.cu", "swept_wave_euler.cu",
+           "swept_band_heat.cu", "swept_band_ks.cu", "swept_band_euler.cu", "alu_peak.cu"]
+HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", "swept_band.cuh", os.path.join("..", "..", "include", "swept1d.h")]
 # -fmad=false: no implicit FMA contraction -- the only fused operations are the explicit fma() calls of the
 # canonical evaluation order, so classic, swept and the CPU oracle round identically.
 # Default -prec-div=true -prec-sqrt=true -ftz=false are kept (IEEE division and square root, denormals).

@@ -24,7 +24,7 @@ struct swept_ctx {
     int device, sm_count, max_smem;
     int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
     void *sync;            // chain kernel: work counter (8 bytes) + done[nx / 8] flags
-    int max_tile_width, tuned_tile_width;
+    int max_tile_width, tuned_tile_width, last_sweep_launch;
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
@@ -107,7 +107,8 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     h->nx = nx; h->dx = dx; h->dt = dt; h->alpha = alpha; h->gamma = gamma;
     h->device = dev;
     h->kernel = SWEPT_KERNEL_WAVE;
-    h->chain = 1;
+    h->chain = 2;
+    h->last_sweep_launch = -1;
     h->warps_per_block = 4;
     h->max_tile_width = p ? p->max_tile_width : 0;
     if (dtype == SWEPT_F64) fill_consts<double>(h); else fill_consts<float>(h);
@@ -300,7 +301,7 @@ static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, in
     };
     auto half_cycles = [&](int w, int64_t q, bool chained) {
         if (q <= 0) return;
-        if (chained) { push(SWEPT_LAUNCH_CHAIN, w, 0, q); return; }
+        if (chained) { push(chain == 2 ? SWEPT_LAUNCH_BAND : SWEPT_LAUNCH_CHAIN, w, 0, q); return; }
         push(SWEPT_LAUNCH_UP, w, 0, 1);
         if (q > 1) push(SWEPT_LAUNCH_DIAMOND, w, w / 2, q - 1);   // offsets W/2, 0, W/2, ...
         push(SWEPT_LAUNCH_DOWN, w, (q & 1) ? w / 2 : 0, 1);
@@ -351,15 +352,23 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
             case SWEPT_LAUNCH_UP: e = launch_phase(h, kernel, MODE_UP, d_u, L.tile_width, L.offset, st); ++*launches; break;
             case SWEPT_LAUNCH_DOWN: e = launch_phase(h, kernel, MODE_DOWN, d_u, L.tile_width, L.offset, st); ++*launches; break;
             case SWEPT_LAUNCH_DIAMOND:
+                h->last_sweep_launch = SWEPT_LAUNCH_DIAMOND;
                 for (int64_t k = 0; k < L.count && e == cudaSuccess; ++k) {
                     const int64_t off = (k & 1) ? (L.offset ? 0 : L.tile_width / 2) : L.offset;
                     e = launch_phase(h, kernel, MODE_DIAMOND, d_u, L.tile_width, off, st);
                     ++*launches;
                 }
                 break;
+            case SWEPT_LAUNCH_BAND:
+                e = launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, st);
+                if (e != cudaErrorNotSupported) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
+                cudaGetLastError();
+                /* the band schedule does not fit this device / size: same half-cycles through the tile-flag kernel */
+                /* fall through */
             case SWEPT_LAUNCH_CHAIN:
                 e = launch_swept_chain(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->warps_per_block,
                                        h->blocks_per_sm, h->sm_count, st);
+                h->last_sweep_launch = SWEPT_LAUNCH_CHAIN;
                 ++*launches;
                 break;
             default: e = cudaErrorInvalidValue;
@@ -481,7 +490,7 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
             h->swept_graph = value;
             return SWEPT_OK;
         case SWEPT_OPT_CHAIN:
-            if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0 or 1");
+            if (value != 0 && value != 1 && value != 2) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0, 1 or 2");
             h->chain = value;
             return SWEPT_OK;
         case SWEPT_OPT_BLOCKS_PER_SM:
@@ -510,6 +519,7 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->launches_total = h->launches_total;
     info->sm_count = h->sm_count;
     info->max_smem_per_block = h->max_smem;
+    info->last_sweep_launch = h->last_sweep_launch;
     return SWEPT_OK;
 }
 

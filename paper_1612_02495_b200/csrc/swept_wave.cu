@@ -9,6 +9,9 @@ namespace swept {
     cudaError_t launch_swept_chain_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                \
                                           const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count, cudaStream_t st);    \
     cudaError_t swept_wave_prepare_##prob(int dtype, int max_smem);                                                             \
+    cudaError_t launch_swept_band_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                 \
+                                         const ConstBlock &cb, int sm_count, int max_smem, cudaStream_t st);                    \
+    cudaError_t swept_band_prepare_##prob(int dtype, int max_smem);                                                             \
     int swept_wave_supports_##prob(int W);
 DECL(heat)
 DECL(ks)
@@ -40,6 +43,13 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
     return launch_swept_chain_euler(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, st);
 }
 
+cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
+                              int sm_count, int max_smem, cudaStream_t st) {
+    if (problem == SWEPT_HEAT) return launch_swept_band_heat(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, st);
+    if (problem == SWEPT_KS) return launch_swept_band_ks(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, st);
+    return launch_swept_band_euler(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, st);
+}
+
 int swept_wave_supports(int problem, int dtype, int W) {
     (void)dtype;
     if (problem == SWEPT_HEAT) return swept_wave_supports_heat(W);
@@ -51,9 +61,17 @@ cudaError_t swept_wave_prepare(int problem, int dtype) {
     int dev = 0, max_smem = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    if (problem == SWEPT_HEAT) return swept_wave_prepare_heat(dtype, max_smem);
-    if (problem == SWEPT_KS) return swept_wave_prepare_ks(dtype, max_smem);
-    return swept_wave_prepare_euler(dtype, max_smem);
+    cudaError_t e;
+    if (problem == SWEPT_HEAT) {
+        if ((e = swept_wave_prepare_heat(dtype, max_smem)) != cudaSuccess) return e;
+        return swept_band_prepare_heat(dtype, max_smem);
+    }
+    if (problem == SWEPT_KS) {
+        if ((e = swept_wave_prepare_ks(dtype, max_smem)) != cudaSuccess) return e;
+        return swept_band_prepare_ks(dtype, max_smem);
+    }
+    if ((e = swept_wave_prepare_euler(dtype, max_smem)) != cudaSuccess) return e;
+    return swept_band_prepare_euler(dtype, max_smem);
 }
 
 }  // namespace swept

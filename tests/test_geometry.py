@@ -140,7 +140,7 @@ class Model:
             elif kind == sw.LAUNCH_DIAMOND:
                 for k in range(count):
                     self.launch("diamond", W, offset if k % 2 == 0 else (0 if offset else W // 2))
-            elif kind == sw.LAUNCH_CHAIN:
+            elif kind in (sw.LAUNCH_CHAIN, sw.LAUNCH_BAND):      # the same phases in one launch (tile flags / streaming bands)
                 for p in range(count + 1):
                     self.launch("up" if p == 0 else ("down" if p == count else "diamond"), W, W // 2 if p & 1 else 0)
             else:
@@ -159,7 +159,7 @@ CASES = [
 ]
 
 
-@pytest.mark.parametrize("chain", [False, True], ids=["per-launch", "chain"])
+@pytest.mark.parametrize("chain", [0, 1, 2], ids=["per-launch", "chain", "band"])
 @pytest.mark.parametrize("problem,nx,W,nsteps", CASES)
 def test_plan_executed_on_the_model_equals_naive_stepping(problem, nx, W, nsteps, chain):
     h, S = sw.RADIUS[problem], sw.STAGES[problem]
@@ -187,6 +187,9 @@ def test_plan_structure_and_launch_counts():
     assert [(k, W) for k, W, _, _ in plan] == [(sw.LAUNCH_UP, 512), (sw.LAUNCH_DOWN, 512), (sw.LAUNCH_UP, 128), (sw.LAUNCH_DOWN, 128),
                                                (sw.LAUNCH_CLASSIC, 0), (sw.LAUNCH_CHAIN, 1024)]
     assert plan[-1][3] == 97 and plan[-2][3] == 16
+    # the default (SWEPT_OPT_CHAIN = 2, streaming bands) differs only in the kind of the last entry
+    band = sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE)
+    assert band[:-1] == plan[:-1] and band[-1] == (sw.LAUNCH_BAND, 1024, 0, 97)
     # q = 0: everything classic or narrower tiles
     assert sw.plan(sw.KS, 4096, 3, 128, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_CLASSIC, 0, 0, 3)]
     assert sw.plan(sw.KS, 4096, 0, 128) == []

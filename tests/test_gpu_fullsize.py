@@ -51,7 +51,7 @@ def test_full_size_bench_configuration(problem, dtype, nx, kind, M):
         W = s.tune(to_dev(u0))                       # what bench.py does: tuned width, chain on (the default)
         assert s.tile_width_ok(W)
         kinds = [k for k, *_ in sw.plan(problem, nx, nsteps, W, dtype=sw.F64 if dtype == np.float64 else sw.F32)]
-        assert kinds[-1] == sw.LAUNCH_CHAIN
+        assert kinds[-1] == sw.LAUNCH_BAND               # the default: streaming bands (runs as CHAIN where they do not fit)
         us, un = to_dev(u0), to_dev(u0)
         s.swept_run(us, nsteps, 0)                   # 0 = the tuned width
         s.naive_run(un, nsteps)
