@@ -107,6 +107,8 @@ typedef struct {
     int max_smem_per_block;      /* opt-in shared-memory limit per block (bytes)                 */
     int last_sweep_launch;       /* SWEPT_LAUNCH_* that ran the half-cycles of the last swept_run enqueued outside a
                                     graph (BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet        */
+    int tuned_chain;             /* SWEPT_OPT_CHAIN value (1 | 2) swept_tune measured as faster for tuned_tile_width under
+                                    the default option 2; 0 = not tuned                                              */
 } swept_info_t;
 
 /* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's
@@ -147,10 +149,23 @@ int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
 int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int tile_width, int kernel, int chain,
                    swept_launch_t *out, int64_t cap);
 
+/* Host logic of the streaming-band schedule (SWEPT_OPT_CHAIN = 2), no device needed.  A band is the chain of tiles that
+ * stitch onto one another's upper-left edge from half-cycle to half-cycle (Fig. 2b); ntiles = nx / tile_width
+ * bands exist.  swept_band_layout: the grid for `ntiles` bands on `sm_count` SMs with `warps_per_block` warps per block (at
+ * most one block per SM).  swept_band_owner: the block, the warp of that block, and the position in that warp's band list
+ * that own `band`: band n goes to sub-partition slot n mod slots, so every slot carries floor or ceil(ntiles / slots) bands. */
+typedef struct {
+    int blocks, warps_per_block, slots_per_block, warps_per_slot, slots, max_bands_per_warp, ntiles;
+} swept_band_layout_t;
+int swept_band_layout(int ntiles, int sm_count, int warps_per_block, swept_band_layout_t *out);
+int swept_band_owner(const swept_band_layout_t *layout, int band, int *block, int *warp, int *index);
+
 /* The paper's best-node-size sweep: time swept_run on d_u_scratch (device,
  * [ncomp][nx], contents destroyed) for every legal tile width (and kernel launch shape) up to
  * max_tile_width with at most blocks_per_sm_cap resident blocks per SM (0 = no cap), keep the
- * fastest in the handle and return it in *best_tile_width (may be NULL).  SYNCHRONISES the stream. */
+ * fastest in the handle and return it in *best_tile_width (may be NULL).  Under the default SWEPT_OPT_CHAIN = 2 each
+ * width is timed with the streaming band kernel and with the tile-flag kernel, and swept_run uses the faster of the two
+ * for the tuned width.  SYNCHRONISES the stream. */
 int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream);
 
 /* End-to-end convenience used for the `e2e` measurement: copy h_u (HOST, [ncomp][nx], ideally

@@ -32,6 +32,7 @@ NCOMP = {HEAT: 1, KS: 1, EULER: 3}
 SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
+    "swept_band_layout", "swept_band_owner",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -53,12 +54,16 @@ class _Info(ctypes.Structure):
         ("problem", ctypes.c_int), ("dtype", ctypes.c_int), ("radius", ctypes.c_int), ("stages", ctypes.c_int), ("ncomp", ctypes.c_int),
         ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
-        ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int),
+        ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int), ("tuned_chain", ctypes.c_int),
     ]
 
 
 class _Launch(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int), ("tile_width", ctypes.c_int), ("offset", ctypes.c_int64), ("count", ctypes.c_int64)]
+
+
+class _BandLayout(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int) for n in ("blocks", "warps_per_block", "slots_per_block", "warps_per_slot", "slots", "max_bands_per_warp", "ntiles")]
 
 
 _lib = None
@@ -92,6 +97,8 @@ def lib() -> ctypes.CDLL:
     L.swept_measure_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     L.swept_destroy.argtypes = [vp]
     L.swept_plan.argtypes = [ci, ci, i64, i64, ci, ci, ci, ctypes.POINTER(_Launch), i64]
+    L.swept_band_layout.argtypes = [ci, ci, ci, ctypes.POINTER(_BandLayout)]
+    L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     for name in SYMBOLS:
         getattr(L, name).restype = ci
     L.swept_plan.restype = i64
@@ -223,6 +230,21 @@ def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F6
     if n < 0:
         _check(int(n))
     return [(buf[i].kind, buf[i].tile_width, buf[i].offset, buf[i].count) for i in range(min(int(n), 64))]
+
+
+def band_layout(ntiles: int, sm_count: int, warps_per_block: int) -> dict:
+    """Grid of the streaming-band schedule (swept_band_layout; host logic, no device needed)."""
+    lay = _BandLayout()
+    _check(lib().swept_band_layout(int(ntiles), int(sm_count), int(warps_per_block), ctypes.byref(lay)))
+    return {n: getattr(lay, n) for n, _ in _BandLayout._fields_}
+
+
+def band_owner(layout: dict, band: int) -> tuple:
+    """(block, warp, index in the warp's band list) that own `band` (swept_band_owner)."""
+    lay = _BandLayout(**layout)
+    b, w, i = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(lib().swept_band_owner(ctypes.byref(lay), int(band), ctypes.byref(b), ctypes.byref(w), ctypes.byref(i)))
+    return b.value, w.value, i.value
 
 
 def steps_per_half_cycle(problem: int, tile_width: int) -> int:

@@ -24,7 +24,7 @@ struct swept_ctx {
     int device, sm_count, max_smem;
     int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
     void *sync;            // chain kernel: work counter (8 bytes) + done[nx / 8] flags
-    int max_tile_width, tuned_tile_width, last_sweep_launch;
+    int max_tile_width, tuned_tile_width, tuned_chain, last_sweep_launch;   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
@@ -340,9 +340,16 @@ static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, i
     return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, h->blocks_per_sm, st);
 }
 
+// The launch-free variant swept_run uses for width W: the option, except that with the default (2 = streaming bands) the
+// tuner's measured choice between the band and the tile-flag kernel is honoured for the width it tuned.
+static int effective_chain(const swept_ctx *h, int W) {
+    if (h->chain == 2 && h->tuned_chain && W == h->tuned_tile_width) return h->tuned_chain;
+    return h->chain;
+}
+
 static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches) {
     swept_launch_t plan[64];   // at most 3 entries per narrower width + 1 classic + 3
-    const int64_t n = build_plan(h->problem, h->dtype, h->nx, nsteps, W, kernel, h->chain, h->max_smem, plan, 64);
+    const int64_t n = build_plan(h->problem, h->dtype, h->nx, nsteps, W, kernel, effective_chain(h, W), h->max_smem, plan, 64);
     if (n > 64) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
     for (int64_t i = 0; i < n && e == cudaSuccess; ++i) {
@@ -388,11 +395,11 @@ extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_w
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int64_t launches = 0;
     if (h->swept_graph && nsteps > 0) {
-        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel && h->sgraph_chain == h->chain;
+        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel && h->sgraph_chain == effective_chain(h, W);
         int64_t l = 0;
         rc = run_graphed(&h->sgraph, reuse, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_swept(h, h->kernel, d_u, nsteps, W, s, n); }, "swept_run(graph)");
         if (rc) return rc;
-        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_chain = h->chain; h->sgraph_launches = l; }
+        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_chain = effective_chain(h, W); h->sgraph_launches = l; }
         launches = h->sgraph_launches;
     } else {
         cudaError_t e = enqueue_swept(h, h->kernel, d_u, nsteps, W, st, &launches);
@@ -417,36 +424,45 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     int wtop = 0;
     for (int W = 4 * h->H; W <= wmax; W <<= 1) if (check_width(h, W, h->kernel, false)) wtop = W;
     if (!wtop) { h->blocks_per_sm = saved_cap; h->swept_graph = saved_graph; return fail(SWEPT_EINVAL, "swept_tune: no legal tile width"); }
-    // every candidate advances the same number of timesteps: four half-cycles of the widest tile
-    const int64_t nsteps = 4 * (int64_t)(wtop / (2 * h->H * h->S));
+    // every candidate advances the same number of timesteps: twelve half-cycles of the widest tile (long enough that the
+    // first and last phase and the one-off wavefront fill of the launch-free kernels do not decide the ranking)
+    const int64_t nsteps = 12 * (int64_t)(wtop / (2 * h->H * h->S));
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    int best = 0;
+    int best = 0, best_chain = 0;
     float best_ms = 1e30f;
     cudaError_t e = cudaSuccess;
+    const int saved_chain = h->chain;
+    h->tuned_chain = 0;
     for (int W = 4 * h->H; W <= wtop && e == cudaSuccess; W <<= 1) {
         if (!check_width(h, W, h->kernel, false)) continue;
-        float ms_min = 1e30f;
-        for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
-            int64_t l = 0;
-            cudaEventRecord(e0, st);
-            e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
-            cudaEventRecord(e1, st);
-            if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-            float ms = 0;
-            if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
-            if (rep > 0 && ms < ms_min) ms_min = ms;
-            h->launches_total += l;
+        // default option (streaming bands): also time the tile-flag kernel, which wins where few warps fit an SM (Euler)
+        for (int mode = saved_chain; mode >= (saved_chain == 2 && h->kernel == SWEPT_KERNEL_WAVE ? 1 : saved_chain) && e == cudaSuccess; --mode) {
+            h->chain = mode;
+            float ms_min = 1e30f;
+            for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
+                int64_t l = 0;
+                cudaEventRecord(e0, st);
+                e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
+                cudaEventRecord(e1, st);
+                if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+                float ms = 0;
+                if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+                if (rep > 0 && ms < ms_min) ms_min = ms;
+                h->launches_total += l;
+            }
+            if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = mode; }
         }
-        if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; }
     }
+    h->chain = saved_chain;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     h->blocks_per_sm = saved_cap;
     h->swept_graph = saved_graph;
     if (e != cudaSuccess) return fail_cuda(e, "swept_tune");
     h->tuned_tile_width = best;
+    h->tuned_chain = (saved_chain == 2 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
     if (best_tile_width) *best_tile_width = best;
     return SWEPT_OK;
 }
@@ -478,7 +494,7 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
     switch (key) {
         case SWEPT_OPT_KERNEL:
             if (value != SWEPT_KERNEL_SMEM && value != SWEPT_KERNEL_WAVE) return fail(SWEPT_EINVAL, "swept_set_option: unknown kernel %d", value);
-            if (value != h->kernel) h->tuned_tile_width = 0;
+            if (value != h->kernel) { h->tuned_tile_width = 0; h->tuned_chain = 0; }
             h->kernel = value;
             return SWEPT_OK;
         case SWEPT_OPT_NAIVE_GRAPH:
@@ -520,6 +536,29 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->sm_count = h->sm_count;
     info->max_smem_per_block = h->max_smem;
     info->last_sweep_launch = h->last_sweep_launch;
+    info->tuned_chain = h->tuned_chain;
+    return SWEPT_OK;
+}
+
+// ---- streaming-band schedule, host logic only (no device needed) ------------------------------------------------
+extern "C" int swept_band_layout(int ntiles, int sm_count, int warps_per_block, swept_band_layout_t *out) {
+    if (!out) return fail(SWEPT_EINVAL, "swept_band_layout: out is NULL");
+    if (ntiles < 1 || sm_count < 1) return fail(SWEPT_EINVAL, "swept_band_layout: ntiles and sm_count must be positive");
+    if (warps_per_block < 1 || warps_per_block > 32 || (warps_per_block > 4 && warps_per_block % 4 != 0))
+        return fail(SWEPT_EINVAL, "swept_band_layout: warps_per_block must be 1, 2, 3, 4 or a multiple of 4 up to 32");
+    const BandGrid g = band_layout(ntiles, sm_count, warps_per_block);
+    out->blocks = g.nblocks; out->warps_per_block = g.wpb; out->slots_per_block = g.SL; out->warps_per_slot = g.wps;
+    out->slots = g.G; out->max_bands_per_warp = g.kmax; out->ntiles = ntiles;
+    return SWEPT_OK;
+}
+
+extern "C" int swept_band_owner(const swept_band_layout_t *lay, int band, int *block, int *warp, int *index) {
+    if (!lay || !block || !warp || !index) return fail(SWEPT_EINVAL, "swept_band_owner: NULL argument");
+    if (band < 0 || band >= lay->ntiles) return fail(SWEPT_EINVAL, "swept_band_owner: band %d outside [0, %d)", band, lay->ntiles);
+    BandGrid g;
+    g.nblocks = lay->blocks; g.wpb = lay->warps_per_block; g.SL = lay->slots_per_block; g.wps = lay->warps_per_slot;
+    g.G = lay->slots; g.kmax = lay->max_bands_per_warp;
+    band_owner(g, band, block, warp, index);
     return SWEPT_OK;
 }
 

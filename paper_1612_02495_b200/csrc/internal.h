@@ -43,6 +43,41 @@ cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t 
 int swept_wave_supports(int problem, int dtype, int W);
 cudaError_t swept_wave_prepare(int problem, int dtype);
 
+// ---- streaming-band schedule (swept_band.cuh): which warp owns which band.  Host logic shared by the kernel, the launch
+// helper and swept_band_layout / swept_band_owner (C ABI, CPU-testable).
+struct BandGrid {
+    int nblocks, wpb, SL, wps, G, kmax;   // blocks, warps per block, sub-partition slots per block (min(wpb, 4)), warps per
+                                          // slot, G = nblocks * SL slots in the grid, kmax = most bands any warp owns
+};
+// Grid for ntiles bands on sm_count SMs with wpb warps per block: one block per SM at most, no more blocks than needed.
+__host__ __device__ inline BandGrid band_layout(int ntiles, int sm_count, int wpb) {
+    BandGrid g;
+    g.wpb = wpb;
+    g.SL = wpb < 4 ? wpb : 4;
+    g.wps = wpb / g.SL;
+    const int nb = (ntiles + wpb - 1) / wpb;
+    g.nblocks = nb < sm_count ? nb : sm_count;
+    g.G = g.nblocks * g.SL;
+    const int stride = g.G * g.wps;
+    g.kmax = (ntiles + stride - 1) / stride;
+    return g;
+}
+// Band n goes to slot n mod G (a slot = the warps of one block that share an SM sub-partition: warp % SL), dealing
+// round n / G to warp (round mod wps) of the slot as its (round / wps)-th band: every slot carries floor or ceil of
+// ntiles / G bands whatever ntiles and the SM count are.
+__host__ __device__ inline int band_first(const BandGrid &g, int block, int warp) { return block * g.SL + warp % g.SL + g.G * (warp / g.SL); }
+__host__ __device__ inline int band_stride(const BandGrid &g) { return g.G * g.wps; }
+__host__ __device__ inline int band_count(const BandGrid &g, int block, int warp, int ntiles) {
+    const int first = band_first(g, block, warp);
+    return first < ntiles ? (ntiles - 1 - first) / band_stride(g) + 1 : 0;
+}
+__host__ __device__ inline void band_owner(const BandGrid &g, int band, int *block, int *warp, int *index) {
+    const int slot = band % g.G, round = band / g.G;
+    *block = slot / g.SL;
+    *warp = slot % g.SL + g.SL * (round % g.wps);
+    *index = round / g.wps;
+}
+
 // FMA-chain microbenchmark (alu_peak.cu)
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st);
 

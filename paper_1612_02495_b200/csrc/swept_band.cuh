@@ -20,8 +20,8 @@
 // floor or ceil(ntiles / G) bands however ntiles and the SM count divide; a warp that owns k > 1 bands runs them
 // phase-major (b_0 p, b_1 p, ..., b_0 p+1, ...) and parks the idle bands' columns in shared memory: at its own first
 // super-row of a tile each lane swaps its PW columns with the parked copy (k - 1 rotating buffers per warp).  Every warp
-// of the grid must be resident (the host sizes the grid by occupancy); waits are on strictly earlier phases of other
-// warps, so the schedule cannot deadlock.
+// of the grid must be resident (the host sizes the grid by occupancy and launches it cooperatively); waits are on
+// strictly earlier phases of other warps, so the schedule cannot deadlock.
 #pragma once
 #include "swept_wave.cuh"
 
@@ -128,10 +128,6 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
     }
 }
 
-struct BandGrid {
-    int nblocks, wpb, SL, wps, G, kmax;                  // SL sub-partition slots per block, wps warps per slot, G = nblocks * SL
-};
-
 template <class P, int PW>
 __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
                                                              BandGrid grid, unsigned *prog, typename P::Consts c) {
@@ -145,9 +141,8 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
     const int64_t mask = nx - 1;
 
     // ---- which bands this warp owns: band n -> slot n % G, round n / G -> warp (round % wps) of the slot, list index round / wps
-    const int slot = (int)blockIdx.x * grid.SL + warp % grid.SL, v = warp / grid.SL;
-    const int first = slot + grid.G * v, stride = grid.G * grid.wps;      // bands first, first + stride, ...
-    const int k = first < ntiles ? (ntiles - 1 - first) / stride + 1 : 0;
+    const int first = band_first(grid, (int)blockIdx.x, warp), stride = band_stride(grid);   // bands first, first + stride, ...
+    const int k = band_count(grid, (int)blockIdx.x, warp, ntiles);
     if (k == 0) return;
     const int n_items = k * (q + 1);
     const int lt_end = n_items * NJI;                     // < 2^31: the host refuses longer runs
@@ -410,16 +405,8 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
         if ((int64_t)sm_count * wpb >= ntiles64) wneed = wpb;
     for (int wpb : cand) {
         if (wpb > wmax || wpb > wneed) continue;
-        BandGrid g;
-        g.wpb = wpb;
-        g.SL = wpb < 4 ? wpb : 4;
-        g.wps = wpb / g.SL;
-        int64_t nb = (ntiles64 + wpb - 1) / wpb;
-        g.nblocks = (int)(nb < sm_count ? nb : sm_count);
-        g.G = g.nblocks * g.SL;
+        const BandGrid g = band_layout(ntiles, sm_count, wpb);
         if (g.G < 2) continue;
-        const int stride = g.G * g.wps;
-        g.kmax = (ntiles + stride - 1) / stride;
         const size_t smem = (size_t)wpb * Gm::warp_values(g.kmax) * sizeof(T);
         if (smem > (size_t)max_smem) continue;
         int per_sm = 0;
@@ -445,8 +432,14 @@ cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, co
     const int ntiles = (int)(nx / Gm::W);
     cudaError_t e = cudaMemsetAsync(sync, 0, sizeof(unsigned) * (size_t)ntiles, st);
     if (e != cudaSuccess) return e;
-    swept_band_kernel<P, PW><<<(unsigned)g.nblocks, g.wpb * 32, smem, st>>>((T *)u, (T *)w, nx, ntiles, (int)q, g, (unsigned *)sync, c);
-    return cudaGetLastError();
+    // Cooperative launch: the warps wait on one another, so the whole grid must be resident at once -- also when another
+    // stream's kernel shares the device (a plain launch could leave two such grids each half scheduled, waiting forever).
+    T *up = (T *)u, *wp = (T *)w;
+    int qi = (int)q, nt = ntiles;
+    unsigned *pr = (unsigned *)sync;
+    typename P::Consts cc = c;
+    void *args[] = {&up, &wp, &nx, &nt, &qi, &g, &pr, &cc};
+    return cudaLaunchCooperativeKernel((const void *)swept_band_kernel<P, PW>, dim3((unsigned)g.nblocks), dim3((unsigned)(g.wpb * 32)), args, smem, st);
 }
 
 template <class P, int PW> cudaError_t band_prepare_pw(int max_smem) {

@@ -203,3 +203,47 @@ def test_plan_rejects_illegal_widths():
         sw.plan(sw.HEAT, 4096, 100, 32, kernel=sw.KERNEL_WAVE)      # WAVE heat starts at W = 64
     with pytest.raises(sw.SweptError):
         sw.plan(sw.HEAT, 1000, 100, 64)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# streaming-band schedule (SWEPT_OPT_CHAIN = 2): host logic of swept_band.cuh through the C ABI, no device needed
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ntiles,sms,wpb", [(2, 148, 1), (64, 148, 1), (1024, 148, 8), (4096, 148, 16), (16384, 148, 8), (8192, 148, 28),
+                                            (4096, 132, 12), (1000, 7, 3), (5, 148, 4)])
+def test_band_assignment_covers_every_band_once_and_balances_the_sub_partitions(ntiles, sms, wpb):
+    lay = sw.band_layout(ntiles, sms, wpb)
+    assert lay["blocks"] <= sms and lay["blocks"] * wpb >= min(ntiles, sms * wpb)          # at most one block per SM
+    assert lay["slots"] == lay["blocks"] * lay["slots_per_block"] and lay["slots_per_block"] * lay["warps_per_slot"] == wpb
+    owners = {}
+    per_slot = {}
+    for band in range(ntiles):
+        b, w, i = sw.band_owner(lay, band)
+        assert 0 <= b < lay["blocks"] and 0 <= w < wpb and 0 <= i < lay["max_bands_per_warp"]
+        assert (b, w, i) not in owners                                                      # one owner position per band
+        owners[(b, w, i)] = band
+        slot = (b, w % lay["slots_per_block"])                                              # warps w, w+SL, ... share a sub-partition
+        per_slot[slot] = per_slot.get(slot, 0) + 1
+    # every warp's list is gap-free (indices 0..k-1) and in band order with a constant stride (the kernel relies on both)
+    by_warp = {}
+    for (b, w, i), band in owners.items():
+        by_warp.setdefault((b, w), {})[i] = band
+    for lst in by_warp.values():
+        assert sorted(lst) == list(range(len(lst)))
+        bands = [lst[i] for i in range(len(lst))]
+        assert all(y - x == lay["slots"] * lay["warps_per_slot"] for x, y in zip(bands, bands[1:]))
+    # neighbouring bands never share a warp (a warp would wait on its own unfinished tile), and the load per sub-partition
+    # slot differs by at most one band
+    if lay["slots"] >= 2:
+        for band in range(ntiles):
+            assert sw.band_owner(lay, band)[:2] != sw.band_owner(lay, (band + 1) % ntiles)[:2] or ntiles < 2
+    loads = list(per_slot.values()) + [0] * (lay["slots"] - len(per_slot))
+    assert max(loads) - min(loads) <= 1
+    assert max(len(l) for l in by_warp.values()) == lay["max_bands_per_warp"]
+
+
+def test_band_layout_rejects_bad_arguments():
+    for args in ((0, 148, 4), (10, 0, 4), (10, 148, 0), (10, 148, 6), (10, 148, 33)):
+        with pytest.raises(sw.SweptError):
+            sw.band_layout(*args)
+    with pytest.raises(sw.SweptError):
+        sw.band_owner(sw.band_layout(8, 4, 2), 8)

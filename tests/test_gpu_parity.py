@@ -285,3 +285,85 @@ def test_chain_graph_replay_and_two_streams():
     assert_bits_equal(u1.cpu().numpy(), ref, "stream 1")
     assert_bits_equal(u2.cpu().numpy(), ref, "stream 2 (graph replay)")
     s1.close(); s2.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# streaming bands (SWEPT_OPT_CHAIN = 2, the default): columns resident across half-cycles, progress counters
+# ------------------------------------------------------------------------------------------------------------
+BAND_CASES = [
+    # problem, dtype, nx, W, q                      what it exercises
+    (wl.HEAT, np.float64, 512, 256, 9),             # two bands, each the other's neighbour on both sides
+    (wl.HEAT, np.float64, 1 << 12, 128, 1),         # q = 1: upright triangle straight into the closing triangle
+    (wl.HEAT, np.float64, 1 << 12, 128, 2),
+    (wl.HEAT, np.float32, 1 << 16, 256, 40),        # one band per warp, many phases (SR = 2 iterations)
+    (wl.HEAT, np.float64, 1 << 22, 1024, 5),        # 4096 bands: warps own 1 or 2 bands, parked columns in shared memory
+    (wl.HEAT, np.float32, 1 << 22, 256, 5),         # 16384 bands: up to 6 bands per warp, rotating parked buffers
+    (wl.HEAT, np.float64, 1 << 21, 128, 6),         # SR = 1 heat tiles, 16384 bands
+    (wl.KS, np.float64, 1 << 14, 256, 11),
+    (wl.KS, np.float32, 1 << 21, 256, 4),           # 8192 bands, several per warp
+    (wl.KS, np.float64, 1 << 20, 1024, 3),
+    (wl.EULER, np.float64, 1 << 13, 256, 7),
+    (wl.EULER, np.float32, 1 << 20, 256, 3),        # 4096 bands on few resident warps
+    (wl.EULER, np.float64, 1 << 18, 512, 2),
+]
+
+
+@pytest.mark.parametrize("problem,dtype,nx,W,q", BAND_CASES)
+def test_band_kernel_equals_classic(problem, dtype, nx, W, q):
+    import torch
+    from gpu_util import BAND
+    w = _noise(problem, nx)
+    nsteps = q * _sph(problem, W) + 3                      # + a remainder that runs before the band launch
+    with solver_for(w, dtype) as s:
+        s.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
+        assert s.tile_width_ok(W)
+        u = to_dev(w.initial(dtype))
+        s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        assert s.info()["last_sweep_launch"] == sw.LAUNCH_BAND, "this case must run on swept_band_kernel, not fall back"
+        got = u.cpu().numpy()
+    assert_bits_equal(got, run_naive(w, dtype, nsteps), f"band nx={nx} W={W} q={q}")
+
+
+def test_band_falls_back_to_tile_flags_where_the_schedule_does_not_fit():
+    """One 32-iteration chunk per tile (heat W = 64) and a single band (nx = W) cannot run as streaming bands: the same
+    half-cycles run on swept_chain_kernel, with the same result."""
+    import torch
+    for nx, W in ((1 << 12, 64), (256, 256)):
+        w = _noise(wl.HEAT, nx)
+        with solver_for(w, np.float64) as s:
+            u = to_dev(w.initial(np.float64))
+            s.swept_run(u, 5 * _sph(wl.HEAT, W), W)
+            torch.cuda.synchronize()
+            assert s.info()["last_sweep_launch"] == sw.LAUNCH_CHAIN
+            assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float64, 5 * _sph(wl.HEAT, W)), f"fallback nx={nx} W={W}")
+
+
+def test_band_repeated_calls_two_streams_and_graph_replay():
+    """Band launches are cooperative (every warp resident): two solvers on two streams, one replaying a CUDA graph."""
+    import torch
+    w = _noise(wl.HEAT, 1 << 20)
+    s1, s2 = solver_for(w, np.float64), solver_for(w, np.float64)
+    s2.set_option(sw.OPT_SWEPT_GRAPH, 1)
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    u1, u2 = to_dev(w.initial(np.float64)), to_dev(w.initial(np.float64))
+    torch.cuda.synchronize()
+    for _ in range(3):
+        s1.swept_run(u1, 1100, 512, stream=st1)
+        s2.swept_run(u2, 1100, 512, stream=st2)
+    torch.cuda.synchronize()
+    assert s1.info()["last_sweep_launch"] == sw.LAUNCH_BAND
+    ref = run_naive(w, np.float64, 3300)
+    assert_bits_equal(u1.cpu().numpy(), ref, "stream 1")
+    assert_bits_equal(u2.cpu().numpy(), ref, "stream 2 (graph replay)")
+    s1.close(); s2.close()
+
+
+def test_tuner_chooses_between_bands_and_tile_flags():
+    w = _noise(wl.EULER, 1 << 16)
+    with solver_for(w, np.float64) as s:
+        W = s.tune(to_dev(w.initial(np.float64)))
+        info = s.info()
+        assert info["tuned_tile_width"] == W and info["tuned_chain"] in (sw.CHAIN_TILES, sw.CHAIN_BANDS)
+        nsteps = 7 * _sph(wl.EULER, W) + 1
+        assert_bits_equal(run_swept(w, np.float64, nsteps, W, (sw.KERNEL_WAVE, info["tuned_chain"])), run_naive(w, np.float64, nsteps), "tuned variant")
