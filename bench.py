@@ -64,6 +64,8 @@ def parse():
     ap.add_argument("--tile-width", type=int, default=0, help="0 = tuned (swept_tune)")
     ap.add_argument("--kernel", default="wave", choices=["wave", "smem"])
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--stress", action="store_true", help="BASELINE.json configs[4]: heat, KS, Euler x fp32, fp64 at nx = 2^22, 100 000 timesteps, "
+                    "every tile width 32..2048 x kernel x resident-blocks cap 1..4 (written to gpurun_out/stress.json / stress.md)")
     ap.add_argument("--variants", default="", help="--sweep: comma list of band,chain,wave,smem (default all)")
     ap.add_argument("--chain", type=int, default=2, choices=[0, 1, 2],
                     help="launch-free sweep: 2 = streaming bands (default), 1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
@@ -280,6 +282,85 @@ def run_sweep(args):
               f"{r['best_value']:.1f} | {r['best']} | {r['speedup_vs_naive']:.1f}x | {r['speedup_vs_naive_graph']:.1f}x |")
 
 
+# ---------------------------------------------------------------------------------------------------------------
+# --stress: BASELINE.json configs[4] -- the tuning sweep at nx = 2^22
+# ---------------------------------------------------------------------------------------------------------------
+def run_stress(args):
+    import torch
+
+    import paper_1612_02495_b200 as sw
+
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    nx = args.nx
+    rows = []
+    for problem in ("heat", "ks", "euler"):
+        for dname in ("f64", "f32"):
+            np_dtype = np.float64 if dname == "f64" else np.float32
+            sw_dtype = sw.F64 if dname == "f64" else sw.F32
+            w = wl.make(problem, nx, "config5")
+            nsteps = args.nsteps or w.nsteps
+            u0 = torch.from_numpy(w.initial(np_dtype)).cuda()
+            u = u0.clone()
+
+            def timed(fn):
+                fn()
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); fn(); e1.record(stream); e1.synchronize()
+                return e0.elapsed_time(e1) * 1e-3
+
+            with sw.Solver(w.problem, nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma) as s:
+                ns_naive = min(nsteps, 1000)
+                s.set_option(sw.OPT_NAIVE_GRAPH, 1)
+                naive = nx * ns_naive / timed(lambda: s.naive_run(u, ns_naive)) / 1e9
+                res = {}
+                for kname, kid, chain, caps in (("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0, 1, 2, 3, 4)),
+                                                ("smem", sw.KERNEL_SMEM, 0, (0, 1, 2, 3, 4))):
+                    s.set_option(sw.OPT_KERNEL, kid)
+                    s.set_option(sw.OPT_CHAIN, chain)
+                    s.set_option(sw.OPT_SWEPT_GRAPH, 1 if kname == "smem" else 0)
+                    for W in (32, 64, 128, 256, 512, 1024, 2048):
+                        if not s.tile_width_ok(W):
+                            continue
+                        for cap in caps:
+                            s.set_option(sw.OPT_BLOCKS_PER_SM, cap)
+                            u.copy_(u0)
+                            # rates do not depend on the step count: a 1000-step probe (also the warm-up) sizes the timed
+                            # run to the config's 100 000 steps or about 1.5 s, whichever is shorter
+                            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            e0.record(stream); s.swept_run(u, 1000, W); e1.record(stream); e1.synchronize()
+                            ns = int(min(nsteps, max(1000, 1000 * 1.5 / max(e0.elapsed_time(e1) * 1e-3, 1e-6))))
+                            u.copy_(u0)
+                            flush.zero_()
+                            e0.record(stream); s.swept_run(u, ns, W); e1.record(stream); e1.synchronize()
+                            t = e0.elapsed_time(e1) * 1e-3
+                            ran = sw.LAUNCH_NAMES.get(s.info()["last_sweep_launch"], "-") if kname != "smem" else "smem"
+                            if kname == "band" and ran != "band":
+                                continue            # the band schedule does not fit: this (W) is the chain row
+                            res[f"{kname}/W={W}/cap={cap}"] = nx * ns / t / 1e9
+                s.set_option(sw.OPT_BLOCKS_PER_SM, 0)
+            best = max(res, key=res.get)
+            rows.append({"problem": problem, "dtype": dname, "nx": nx, "nsteps": nsteps, "classic_graph": naive, "results": res, "best": best,
+                         "best_value": res[best]})
+            print(f"# {problem} {dname}: classic(graph) {naive:.1f}  best {best} {res[best]:.1f} GPts*steps/s", file=sys.stderr, flush=True)
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "stress.json"), "w") as f:
+        json.dump({"unit": "GPts*steps/s", "rows": rows}, f, indent=1)
+    print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: band | chain (W, cap) | smem (W, cap) |")
+    print("|---|---|---:|---:|---|---:|---|---|---|")
+    for r in rows:
+        def bk(k):
+            c = {n: v for n, v in r["results"].items() if n.startswith(k + "/")}
+            if not c:
+                return "-"
+            b = max(c, key=c.get)
+            return f"{c[b]:.1f} ({b.split('/', 1)[1]})"
+        print(f"| {r['problem']} | {r['dtype']} | {r['classic_graph']:.1f} | {r['best_value']:.1f} | {r['best']} | {r['best_value'] / r['classic_graph']:.1f}x | "
+              f"{bk('band')} | {bk('chain')} | {bk('smem')} |")
+
+
 def main():
     args = parse()
     if args.impl == "reference":
@@ -287,6 +368,9 @@ def main():
         return
     if args.sweep:
         run_sweep(args)
+        return
+    if args.stress:
+        run_stress(args)
         return
 
     import torch

@@ -109,6 +109,8 @@ typedef struct {
                                     graph (BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet        */
     int tuned_chain;             /* SWEPT_OPT_CHAIN value (1 | 2) swept_tune measured as faster for tuned_tile_width under
                                     the default option 2; 0 = not tuned                                              */
+    int tuned_blocks_per_sm;     /* resident-blocks cap swept_tune measured as fastest for tuned_tile_width when called with
+                                    blocks_per_sm_cap = 0 (0 = none); used while SWEPT_OPT_BLOCKS_PER_SM is 0          */
 } swept_info_t;
 
 /* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's
@@ -165,7 +167,8 @@ int swept_band_owner(const swept_band_layout_t *layout, int band, int *block, in
  * max_tile_width with at most blocks_per_sm_cap resident blocks per SM (0 = no cap), keep the
  * fastest in the handle and return it in *best_tile_width (may be NULL).  Under the default SWEPT_OPT_CHAIN = 2 each
  * width is timed with the streaming band kernel and with the tile-flag kernel, and swept_run uses the faster of the two
- * for the tuned width.  SYNCHRONISES the stream. */
+ * for the tuned width; with blocks_per_sm_cap = 0 the register-resident per-tile kernels are also timed at 4, 3 and 2 blocks
+ * of 4 warps per SM (the paper's occupancy trade-off).  SYNCHRONISES the stream. */
 int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream);
 
 /* End-to-end convenience used for the `e2e` measurement: copy h_u (HOST, [ncomp][nx], ideally

@@ -24,7 +24,7 @@ struct swept_ctx {
     int device, sm_count, max_smem;
     int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
     void *sync;            // chain kernel: work counter (8 bytes) + done[nx / 8] flags
-    int max_tile_width, tuned_tile_width, tuned_chain, last_sweep_launch;   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
+    int max_tile_width, tuned_tile_width, tuned_chain, tuned_cap, last_sweep_launch;   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
@@ -335,9 +335,11 @@ extern "C" int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps
     return build_plan(problem, dtype, nx, nsteps, tile_width, kernel, chain, SWEPT_SMEM_LIMIT_B200, out, cap);
 }
 
+static int effective_cap(const swept_ctx *h, int W);
+
 static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, int W, int64_t offset, cudaStream_t st) {
     if (kernel == SWEPT_KERNEL_SMEM) return launch_swept_smem(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, st);
-    return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, h->blocks_per_sm, st);
+    return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, effective_cap(h, W), st);
 }
 
 // The launch-free variant swept_run uses for width W: the option, except that with the default (2 = streaming bands) the
@@ -345,6 +347,12 @@ static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, i
 static int effective_chain(const swept_ctx *h, int W) {
     if (h->chain == 2 && h->tuned_chain && W == h->tuned_tile_width) return h->tuned_chain;
     return h->chain;
+}
+
+// Resident-blocks cap for width W: the option if set, else the cap the tuner measured as fastest for the tuned width.
+static int effective_cap(const swept_ctx *h, int W) {
+    if (h->blocks_per_sm == 0 && h->tuned_cap && W == h->tuned_tile_width) return h->tuned_cap;
+    return h->blocks_per_sm;
 }
 
 static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches) {
@@ -374,7 +382,7 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
                 /* fall through */
             case SWEPT_LAUNCH_CHAIN:
                 e = launch_swept_chain(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->warps_per_block,
-                                       h->blocks_per_sm, h->sm_count, st);
+                                       effective_cap(h, L.tile_width), h->sm_count, st);
                 h->last_sweep_launch = SWEPT_LAUNCH_CHAIN;
                 ++*launches;
                 break;
@@ -430,29 +438,39 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    int best = 0, best_chain = 0;
+    int best = 0, best_chain = 0, best_cap = 0;
     float best_ms = 1e30f;
     cudaError_t e = cudaSuccess;
     const int saved_chain = h->chain;
     h->tuned_chain = 0;
+    h->tuned_cap = 0;
+    const bool wave = h->kernel == SWEPT_KERNEL_WAVE;
     for (int W = 4 * h->H; W <= wtop && e == cudaSuccess; W <<= 1) {
         if (!check_width(h, W, h->kernel, false)) continue;
         // default option (streaming bands): also time the tile-flag kernel, which wins where few warps fit an SM (Euler)
-        for (int mode = saved_chain; mode >= (saved_chain == 2 && h->kernel == SWEPT_KERNEL_WAVE ? 1 : saved_chain) && e == cudaSuccess; --mode) {
+        for (int mode = saved_chain; mode >= (saved_chain == 2 && wave ? 1 : saved_chain) && e == cudaSuccess; --mode) {
             h->chain = mode;
-            float ms_min = 1e30f;
-            for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
-                int64_t l = 0;
-                cudaEventRecord(e0, st);
-                e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
-                cudaEventRecord(e1, st);
-                if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-                float ms = 0;
-                if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
-                if (rep > 0 && ms < ms_min) ms_min = ms;
-                h->launches_total += l;
+            // resident warps per SM: with no cap given, the register-resident kernels (other than the band kernel, which sizes
+            // its own grid) are also tried at 4, 3 and 2 blocks of 4 warps per SM -- fp32 and KS run faster below full occupancy
+            static const int caps_auto[] = {0, 4, 3, 2};
+            const int ncaps = (blocks_per_sm_cap == 0 && wave && mode != 2) ? 4 : 1;
+            for (int ci = 0; ci < ncaps && e == cudaSuccess; ++ci) {
+                const int cap = ncaps == 1 ? blocks_per_sm_cap : caps_auto[ci];
+                h->blocks_per_sm = cap;
+                float ms_min = 1e30f;
+                for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
+                    int64_t l = 0;
+                    cudaEventRecord(e0, st);
+                    e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
+                    cudaEventRecord(e1, st);
+                    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+                    float ms = 0;
+                    if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+                    if (rep > 0 && ms < ms_min) ms_min = ms;
+                    h->launches_total += l;
+                }
+                if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = mode; best_cap = cap; }
             }
-            if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = mode; }
         }
     }
     h->chain = saved_chain;
@@ -463,6 +481,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     if (e != cudaSuccess) return fail_cuda(e, "swept_tune");
     h->tuned_tile_width = best;
     h->tuned_chain = (saved_chain == 2 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
+    h->tuned_cap = blocks_per_sm_cap == 0 ? best_cap : 0;
     if (best_tile_width) *best_tile_width = best;
     return SWEPT_OK;
 }
@@ -494,7 +513,7 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
     switch (key) {
         case SWEPT_OPT_KERNEL:
             if (value != SWEPT_KERNEL_SMEM && value != SWEPT_KERNEL_WAVE) return fail(SWEPT_EINVAL, "swept_set_option: unknown kernel %d", value);
-            if (value != h->kernel) { h->tuned_tile_width = 0; h->tuned_chain = 0; }
+            if (value != h->kernel) { h->tuned_tile_width = 0; h->tuned_chain = 0; h->tuned_cap = 0; }
             h->kernel = value;
             return SWEPT_OK;
         case SWEPT_OPT_NAIVE_GRAPH:
@@ -537,6 +556,7 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->max_smem_per_block = h->max_smem;
     info->last_sweep_launch = h->last_sweep_launch;
     info->tuned_chain = h->tuned_chain;
+    info->tuned_blocks_per_sm = h->tuned_cap;
     return SWEPT_OK;
 }
 

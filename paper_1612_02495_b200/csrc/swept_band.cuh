@@ -23,6 +23,8 @@
 // of the grid must be resident (the host sizes the grid by occupancy and launches it cooperatively); waits are on
 // strictly earlier phases of other warps, so the schedule cannot deadlock.
 #pragma once
+#include <type_traits>
+
 #include "swept_wave.cuh"
 
 namespace swept {
@@ -53,6 +55,8 @@ template <class P, int PW> constexpr int band_max_threads() {
     const int est = P::NC * (2 * P::H + PW) * (int)(sizeof(typename P::real) / 4) + (P::GROUPED ? 110 : 56 + 16 * (P::H - 1));
     int warps = 65536 / (32 * est);
     warps = warps >= 4 ? (warps & ~3) : (warps < 1 ? 1 : warps);
+    // KS fp64 at 32 points per lane spills at the 170 registers 12 warps leave; 8 warps with up to 255 registers run faster
+    if (P::H == 2 && !P::GROUPED && sizeof(typename P::real) == 8 && PW == 32) warps = 8;
     return 32 * (warps > 32 ? 32 : warps);
 }
 
@@ -184,6 +188,28 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
         hi = p_cur == q ? L : 0x7fffffff;
         interior = p_cur > 0 && p_cur < q;
     };
+    // This lane enters tile s >= 1 of a warp that owns k > 1 bands: swap its PW columns with the parked copy of the incoming
+    // band (transition s-1 uses buffer (s-1) mod (k-1)), and hand the incoming band's last D columns -- before this lane's
+    // first super-row changes them -- to lane l+1, which swaps one iteration later.
+    auto swap_bands = [&](int s) {
+        T *buf = col + (size_t)((s - 1) % (k - 1)) * Gm::COL;
+#pragma unroll
+        for (int kk = 0; kk < NC; ++kk)
+#pragma unroll
+            for (int i = 0; i < PW; ++i) {
+                T *a = buf + kk * CS + lane * (PW + 1) + i;
+                const T t = *a;
+                *a = X[kk][D + i];
+                X[kk][D + i] = t;
+            }
+#pragma unroll
+        for (int kk = 0; kk < NC; ++kk)
+#pragma unroll
+            for (int d = 0; d < D; ++d) {
+                edge[(kk * 32 + lane) * D + d] = X[kk][PW + d];
+                if (lane > 0) X[kk][d] = edge[(kk * 32 + lane - 1) * D + d];
+            }
+    };
     T keep[SR][NC][D];                                   // this lane's row values after each super-row of its last iteration
 #pragma unroll
     for (int sr = 0; sr < SR; ++sr)
@@ -249,42 +275,53 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
         }
 
         // ---- the chunk's 32 iterations.  Steady chunk: every lane is, for the whole chunk, inside diamond tiles (the tiles
-        // of local times K0-31 and K0+31 are both diamond phases) and no lane swaps bands -- nothing depends on the phase.
-        bool steady = K0 >= 31 && K0 + 31 < lt_end && (k == 1 || (K0 & (NJI - 1)) != 0);
+        // of local times K0-31 and K0+31 are both diamond phases) -- nothing depends on the phase; in the first chunk of a tile
+        // the lanes of a warp with k > 1 bands swap columns, each at its own iteration.
+        bool steady = K0 >= 31 && K0 + 31 < lt_end;
+        const bool swapchunk = k > 1 && (K0 & (NJI - 1)) == 0;
         if (steady) {
             const int pa = ((K0 - 31) / NJI) / k, pb = ((K0 + 31) / NJI) / k;
             steady = pa > 0 && pb < q;
         }
         if (steady) {
-            int J = (K0 - lane) & (NJI - 1);
-            const T *fp = feed;
-            T *op = outr + ((K0 - 31) & 63) * SR * D;     // lane 31's slot of local time K0 - 31
-            for (int it = 0; it < 32; ++it) {
-                T recv[SR][NC][D];
-#pragma unroll
-                for (int sr = 0; sr < SR; ++sr)
-#pragma unroll
-                    for (int kk = 0; kk < NC; ++kk)
-#pragma unroll
-                        for (int rho = 0; rho < D; ++rho) {
-                            const T f = fp[(kk * 32 * SR + sr) * D + rho];
-                            const T r = shfl_up1(keep[sr][kk][rho]);
-                            recv[sr][kk][rho] = lane == 0 ? f : r;
-                        }
-                band_super_rows<P, PW, SR, true>(X, recv, keep, c, lane * NP + SR * J + 1, 0, 0);
-                if (lane == 31) {
+            // two instances of the loop: the chunk in which lanes swap bands carries the swap and a warp barrier per iteration,
+            // the others (7 of 8 at W = 1024) stay free of both
+            auto steady_chunk = [&](auto swap_tag) {
+                constexpr bool SWAP = decltype(swap_tag)::value;
+                int J = (K0 - lane) & (NJI - 1);
+                const T *fp = feed;
+                T *op = outr + ((K0 - 31) & 63) * SR * D;     // lane 31's slot of local time K0 - 31
+                for (int it = 0; it < 32; ++it) {
+                    T recv[SR][NC][D];
 #pragma unroll
                     for (int sr = 0; sr < SR; ++sr)
 #pragma unroll
                         for (int kk = 0; kk < NC; ++kk)
 #pragma unroll
-                            for (int rho = 0; rho < D; ++rho) op[(kk * 64 * SR + sr) * D + rho] = keep[sr][kk][rho];
+                            for (int rho = 0; rho < D; ++rho) {
+                                const T f = fp[(kk * 32 * SR + sr) * D + rho];
+                                const T r = shfl_up1(keep[sr][kk][rho]);
+                                recv[sr][kk][rho] = lane == 0 ? f : r;
+                            }
+                    if (SWAP && J == 0) swap_bands((K0 + it - lane) / NJI);
+                    band_super_rows<P, PW, SR, true>(X, recv, keep, c, lane * NP + SR * J + 1, 0, 0);
+                    if (lane == 31) {
+#pragma unroll
+                        for (int sr = 0; sr < SR; ++sr)
+#pragma unroll
+                            for (int kk = 0; kk < NC; ++kk)
+#pragma unroll
+                                for (int rho = 0; rho < D; ++rho) op[(kk * 64 * SR + sr) * D + rho] = keep[sr][kk][rho];
+                    }
+                    J = (J + 1) & (NJI - 1);
+                    fp += SR * D;
+                    op += SR * D;
+                    if (op == outr + 64 * SR * D) op = outr;
+                    if (SWAP) __syncwarp();               // lane l+1 reads the hand-over slot lane l wrote this iteration
                 }
-                J = (J + 1) & (NJI - 1);
-                fp += SR * D;
-                op += SR * D;
-                if (op == outr + 64 * SR * D) op = outr;
-            }
+            };
+            if (swapchunk) steady_chunk(std::true_type{});
+            else steady_chunk(std::false_type{});
             continue;
         }
         {
@@ -315,26 +352,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
                 // ---- this lane enters a new tile: update its phase; with k > 1 swap columns with the parked band
                 const int s = lt / NJI;
                 set_phase(s);
-                if (k > 1 && s > 0) {
-                    T *buf = col + (size_t)((s - 1) % (k - 1)) * Gm::COL;
-#pragma unroll
-                    for (int kk = 0; kk < NC; ++kk)
-#pragma unroll
-                        for (int i = 0; i < PW; ++i) {
-                            T *a = buf + kk * CS + lane * (PW + 1) + i;
-                            const T t = *a;
-                            *a = X[kk][D + i];
-                            X[kk][D + i] = t;
-                        }
-                    // the last D columns of the incoming band's initial state go to lane l+1 (which swaps one iteration later)
-#pragma unroll
-                    for (int kk = 0; kk < NC; ++kk)
-#pragma unroll
-                        for (int d = 0; d < D; ++d) {
-                            edge[(kk * 32 + lane) * D + d] = X[kk][PW + d];
-                            if (lane > 0) X[kk][d] = edge[(kk * 32 + lane - 1) * D + d];
-                        }
-                }
+                if (k > 1 && s > 0) swap_bands(s);
             }
             const bool fed = lane == 0 && p_cur > 0;
 #pragma unroll
