@@ -219,8 +219,13 @@ __device__ __forceinline__ void st_release_gpu(unsigned *p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
+// Launch bounds of the tile-flag kernel: Euler fp64 at 8 points per lane fits 170 registers, which lets a third block of
+// 4 warps onto an SM (the Euler kernels are bound by resident warps); everything else keeps 256 x 1.
+template <class P, int PW> constexpr int chain_max_threads() { return (P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8) ? 128 : 256; }
+template <class P, int PW> constexpr int chain_min_blocks() { return (P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8) ? 3 : 1; }
+
 template <class P, int PW>
-__global__ void __launch_bounds__(256) swept_chain_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
+__global__ void __launch_bounds__((chain_max_threads<P, PW>()), (chain_min_blocks<P, PW>())) swept_chain_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
                                                            unsigned long long *counter, unsigned *done, typename P::Consts c) {
     using T = typename P::real;
     constexpr int W = 32 * PW;
@@ -284,7 +289,7 @@ cudaError_t wave_chain_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, c
     constexpr int W = 32 * PW;
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
     const int ntiles = (int)(nx / W);
-    if (wpb > 8) wpb = 8;
+    if (wpb > chain_max_threads<P, PW>() / 32) wpb = chain_max_threads<P, PW>() / 32;
     while (wpb > 1 && (int64_t)wpb * sm_count > ntiles) wpb >>= 1;   // few tiles: spread the warps over the SMs
     size_t smem = (size_t)wpb * P::NC * W * sizeof(T);
     if (smem < smem_floor) smem = smem_floor;
