@@ -70,6 +70,7 @@ def parse():
     ap.add_argument("--chain", type=int, default=2, choices=[0, 1, 2],
                     help="launch-free sweep: 2 = streaming bands (default), 1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
     ap.add_argument("--no-chain", action="store_true", help="same as --chain 0")
+    ap.add_argument("--blocks-per-sm", type=int, default=0, help="SWEPT_OPT_BLOCKS_PER_SM for the per-tile kernels (0 = none / tuned)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
     return ap.parse_args()
@@ -395,6 +396,8 @@ def main():
     s.set_option(sw.OPT_KERNEL, kernel)
     chain_opt = 0 if args.no_chain else args.chain
     s.set_option(sw.OPT_CHAIN, chain_opt)
+    if args.blocks_per_sm:
+        s.set_option(sw.OPT_BLOCKS_PER_SM, args.blocks_per_sm)
     if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512, 1024)):
         kernel = sw.KERNEL_SMEM
         s.set_option(sw.OPT_KERNEL, kernel)
