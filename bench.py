@@ -63,6 +63,8 @@ def parse():
     ap.add_argument("--nsteps", type=int, default=0, help="timesteps per bench step (0 = the config's count)")
     ap.add_argument("--tile-width", type=int, default=0, help="0 = tuned (swept_tune)")
     ap.add_argument("--kernel", default="wave", choices=["wave", "smem"])
+    ap.add_argument("--boundary", default="periodic", choices=["periodic", "insulated"],
+                    help="insulated: the paper's own heat problem, a rod with insulated ends (heat only; SURVEY.md section 8(f) NEXT-2)")
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--stress", action="store_true", help="BASELINE.json configs[4]: heat, KS, Euler x fp32, fp64 at nx = 2^22, 100 000 timesteps, "
                     "every tile width 32..2048 x kernel x resident-blocks cap 1..4 (written to gpurun_out/stress.json / stress.md)")
@@ -77,7 +79,9 @@ def parse():
 
 
 def workload(args) -> wl.Workload:
-    w = wl.make(args.problem, args.nx, "config")
+    w = wl.heat_rod(args.nx) if args.boundary == "insulated" else wl.make(args.problem, args.nx, "config")
+    if args.boundary == "insulated":
+        w.nsteps = 50_000                          # config 2's step count on the rod
     if args.nsteps:
         w.nsteps = args.nsteps
     return w
@@ -155,16 +159,17 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------------------
 # CPU baseline / reference arm: the oracle as it stands, on the host cores, bounded sample
 # ---------------------------------------------------------------------------------------------------------------
-def oracle_rate(w: wl.Workload, dtype, budget_s: float = 15.0):
+def oracle_rate(w: wl.Workload, dtype, budget_s: float = 15.0, insulated: bool = False):
     import oracle
     u0 = w.initial(dtype)
-    oracle.run(w.problem, u0, 2, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)      # thread start-up, page faults
+    kw = dict(dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma, insulated=insulated)
+    oracle.run(w.problem, u0, 2, **kw)      # thread start-up, page faults
     t0 = time.perf_counter()
-    oracle.run(w.problem, u0, 8, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    oracle.run(w.problem, u0, 8, **kw)
     t8 = time.perf_counter() - t0
     n = int(max(8, min(w.nsteps, budget_s / max(t8 / 8, 1e-9))))
     t0 = time.perf_counter()
-    oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    oracle.run(w.problem, u0, n, **kw)
     dt = time.perf_counter() - t0
     return w.nx * n / dt, n, dt, oracle.num_threads()
 
@@ -178,16 +183,17 @@ def run_reference(args):
     dtype = np.float64 if args.dtype == "f64" else np.float32
     import oracle
     u0 = w.initial(dtype)
+    okw = dict(dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma, insulated=args.boundary == "insulated")
     t0 = time.perf_counter()
-    oracle.run(w.problem, u0, 2, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+    oracle.run(w.problem, u0, 2, **okw)
     per = (time.perf_counter() - t0) / 2
     total = max(1, args.steps + args.warmup)
     n = int(max(2, min(w.nsteps, (90.0 / total) / max(per, 1e-9))))    # whole run <= ~1.5 min
     for _ in range(args.warmup):
-        oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+        oracle.run(w.problem, u0, n, **okw)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.run(w.problem, u0, n, dx=w.dx, dt=w.dt, alpha=w.alpha, gamma=w.gamma)
+        oracle.run(w.problem, u0, n, **okw)
     el = time.perf_counter() - t0
     val = w.nx * n * args.steps / el / 1e9
     sample = f"{n} of the config's {w.nsteps} timesteps per step at nx={w.nx} (rate is step-count independent)"
@@ -392,7 +398,8 @@ def main():
     np_dtype = np.float64 if args.dtype == "f64" else np.float32
     sw_dtype = sw.F64 if args.dtype == "f64" else sw.F32
     kernel = sw.KERNEL_WAVE if args.kernel == "wave" else sw.KERNEL_SMEM
-    s = sw.Solver(w.problem, w.nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma)
+    s = sw.Solver(w.problem, w.nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma,
+                  boundary=sw.BC_INSULATED if args.boundary == "insulated" else sw.BC_PERIODIC)
     s.set_option(sw.OPT_KERNEL, kernel)
     chain_opt = 0 if args.no_chain else args.chain
     s.set_option(sw.OPT_CHAIN, chain_opt)
@@ -531,7 +538,7 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        rate, n, el, cores = oracle_rate(w, np_dtype)
+        rate, n, el, cores = oracle_rate(w, np_dtype, insulated=args.boundary == "insulated")
         cpu = {"value": rate / 1e9, "unit": "GPts*steps/s", "cores": cores, "kind": "oracle",
                "sample": f"{n} of {w.nsteps} timesteps at nx={w.nx} ({el:.1f} s)"}
 
@@ -540,9 +547,9 @@ def main():
         "warmup": max(args.warmup, 3), "ms_per_step": t_dev_max / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {
-            "workload": f"BASELINE.json configs[1]: {w.name}, FTCS periodic r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
+            "workload": f"BASELINE.json configs[1]: {w.name}, FTCS {args.boundary} r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
                         f"{w.nsteps} timesteps per step" if args.problem == "heat" else f"{w.name} nx={w.nx} {w.nsteps} timesteps per step",
-            "nx": w.nx, "nsteps_per_step": w.nsteps, "tile_width": W, "kernel": (("band" if band else "chain") if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
+            "nx": w.nx, "nsteps_per_step": w.nsteps, "boundary": args.boundary, "tile_width": W, "kernel": (("band" if band else "chain") if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
         },

@@ -41,6 +41,13 @@ enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2 };
 /* dtype -- the paper's compile-time REAL as a run-time choice */
 enum { SWEPT_F32 = 0, SWEPT_F64 = 1 };
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_ENOMEM = -2, SWEPT_ECUDA = -3 };
+/* boundary -- SWEPT_BC_PERIODIC: neighbours mod nx (every BASELINE.json config).
+ *             SWEPT_BC_INSULATED (heat only): the paper's heat problem, a rod with insulated ends (Eq. 9
+ *             PAPER.md:266-269): the ghost value beyond an end is the adjacent interior value, T_0 = T_1.  On the shifted
+ *             half-cycles the tile that is "split across the spatial boundary" becomes two tiles, one per end,
+ *             each evaluated on the mirror image of its half (WAVE kernels; the band schedule needs a periodic domain, so the
+ *             launch-free sweep runs on the tile-flag kernel). */
+enum { SWEPT_BC_PERIODIC = 0, SWEPT_BC_INSULATED = 1 };
 
 /* Which swept kernels swept_run uses (SWEPT_OPT_KERNEL):
  *   SWEPT_KERNEL_SMEM  the paper's design (Fig. 5): one block per tile, one
@@ -94,6 +101,7 @@ typedef struct {
     double alpha;       /* heat: thermal diffusivity (Fo = alpha dt / dx^2)       */
     double gamma;       /* Euler: ratio of specific heats                                      */
     int max_tile_width; /* upper bound for the tuner's tile-width sweep, 0 = library default   */
+    int boundary;       /* SWEPT_BC_PERIODIC (0, default) | SWEPT_BC_INSULATED (heat only)      */
 } swept_params_t;
 
 typedef struct {
@@ -107,6 +115,7 @@ typedef struct {
     int max_smem_per_block;      /* opt-in shared-memory limit per block (bytes)                 */
     int last_sweep_launch;       /* SWEPT_LAUNCH_* that ran the half-cycles of the last swept_run enqueued outside a
                                     graph (BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet        */
+    int boundary;                /* SWEPT_BC_*                                                    */
     int tuned_chain;             /* SWEPT_OPT_CHAIN value (1 | 2) swept_tune measured as faster for tuned_tile_width under
                                     the default option 2; 0 = not tuned                                              */
     int tuned_blocks_per_sm;     /* resident-blocks cap swept_tune measured as fastest for tuned_tile_width when called with

@@ -26,6 +26,9 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, f"oracle_heat_{suf}")
             f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double]
             f.restype = ctypes.c_int
+            f = getattr(L, f"oracle_heat_insulated_{suf}")
+            f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+            f.restype = ctypes.c_int
             f = getattr(L, f"oracle_ks_{suf}")
             f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double]
             f.restype = ctypes.c_int
@@ -63,6 +66,15 @@ def heat(u: np.ndarray, nsteps: int, alpha: float, dx: float, dt: float) -> np.n
     return a
 
 
+def heat_insulated(u: np.ndarray, nsteps: int, alpha: float, dx: float, dt: float) -> np.ndarray:
+    """FTCS heat on a rod with insulated ends (Eq. 9, reading G7: ghost = adjacent interior value)."""
+    a, p, nx, suf = _prep(u, 1)
+    rc = getattr(lib(), f"oracle_heat_insulated_{suf}")(p, nx, int(nsteps), float(alpha), float(dx), float(dt))
+    if rc != 0:
+        raise RuntimeError(f"oracle_heat_insulated failed rc={rc}")
+    return a
+
+
 def ks(u: np.ndarray, nsteps: int, dx: float, dt: float) -> np.ndarray:
     """Kuramoto-Sivashinsky, Eq. (4) + (15) + (16) PAPER.md:64, 291, 295, periodic."""
     a, p, nx, suf = _prep(u, 1)
@@ -83,10 +95,11 @@ def euler(U: np.ndarray, nsteps: int, gamma: float, dx: float, dt: float, check_
     return a
 
 
-def run(problem: int, u: np.ndarray, nsteps: int, *, dx: float, dt: float, alpha: float = 1.0, gamma: float = 1.4) -> np.ndarray:
+def run(problem: int, u: np.ndarray, nsteps: int, *, dx: float, dt: float, alpha: float = 1.0, gamma: float = 1.4,
+        insulated: bool = False) -> np.ndarray:
     """Dispatch on the problem id (0 heat, 1 KS, 2 Euler); arrays are [ncomp, nx]."""
     if problem == 0:
-        return heat(u, nsteps, alpha, dx, dt)
+        return heat_insulated(u, nsteps, alpha, dx, dt) if insulated else heat(u, nsteps, alpha, dx, dt)
     if problem == 1:
         return ks(u, nsteps, dx, dt)
     if problem == 2:

@@ -13,6 +13,8 @@
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): heat -- amplification factor 1-4r sin^2(k dx/2),
  * Pascal-triangle delta response (exact), Nyquist annihilation, sum conservation, max principle;
+ * heat with insulated ends -- bitwise equal to the periodic oracle on the mirrored 2n-point rod, cosine
+ * (DCT-II) modes decay by 1-4r sin^2(k pi/2n), exact dyadic hand-stepped 4-point rod, sum conservation;
  * KS -- uniform fixed point, sum conservation, linearised complex growth factor about a uniform
  * offset (pins every coefficient and sign incl. the nonlinear one), bitwise shift equivariance,
  * exact-rational nx=8 hand stepping; Euler -- conservation, uniform fixed point, mirror symmetry,

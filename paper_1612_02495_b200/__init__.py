@@ -21,6 +21,7 @@ KERNEL_SMEM, KERNEL_WAVE = 0, 1
 OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN = 0, 1, 2, 3, 4, 5
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND = 0, 1, 2, 3, 4, 5
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band"}
+BC_PERIODIC, BC_INSULATED = 0, 1
 CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS = 0, 1, 2     # values of OPT_CHAIN (include/swept1d.h); CHAIN_BANDS is the default
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
@@ -46,7 +47,8 @@ class SweptError(RuntimeError):
 
 
 class _Params(ctypes.Structure):
-    _fields_ = [("dtype", ctypes.c_int), ("alpha", ctypes.c_double), ("gamma", ctypes.c_double), ("max_tile_width", ctypes.c_int)]
+    _fields_ = [("dtype", ctypes.c_int), ("alpha", ctypes.c_double), ("gamma", ctypes.c_double), ("max_tile_width", ctypes.c_int),
+                ("boundary", ctypes.c_int)]
 
 
 class _Info(ctypes.Structure):
@@ -54,7 +56,7 @@ class _Info(ctypes.Structure):
         ("problem", ctypes.c_int), ("dtype", ctypes.c_int), ("radius", ctypes.c_int), ("stages", ctypes.c_int), ("ncomp", ctypes.c_int),
         ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
-        ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int), ("tuned_chain", ctypes.c_int), ("tuned_blocks_per_sm", ctypes.c_int),
+        ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int), ("boundary", ctypes.c_int), ("tuned_chain", ctypes.c_int), ("tuned_blocks_per_sm", ctypes.c_int),
     ]
 
 
@@ -142,12 +144,12 @@ class Solver:
     ncomp == 1), contiguous, of the handle's dtype; they are advanced IN PLACE and asynchronously on `stream`."""
 
     def __init__(self, problem, nx: int, dx: float, dt: float, *, dtype=F64, alpha: float = 1.0, gamma: float = 1.4,
-                 max_tile_width: int = 0):
+                 max_tile_width: int = 0, boundary: int = 0):
         if isinstance(problem, str):
             problem = PROBLEMS[problem]
         self._h = ctypes.c_void_p()
         self.problem, self.nx, self.dtype = int(problem), int(nx), _dtype_id(dtype)
-        p = _Params(self.dtype, float(alpha), float(gamma), int(max_tile_width))
+        p = _Params(self.dtype, float(alpha), float(gamma), int(max_tile_width), int(boundary))
         _check(lib().swept_create(ctypes.byref(self._h), self.problem, self.nx, float(dx), float(dt), ctypes.byref(p)))
 
     # -- marshalling ----------------------------------------------------------------------------------------

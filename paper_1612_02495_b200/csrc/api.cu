@@ -14,7 +14,7 @@
 using namespace swept;
 
 struct swept_ctx {
-    int problem, dtype, H, S, NC;
+    int problem, dtype, H, S, NC, bc;
     int64_t nx;
     double dx, dt, alpha, gamma;
     ConstBlock cb;
@@ -95,6 +95,10 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     if (problem == SWEPT_HEAT && !(isfinite(alpha) && alpha > 0.0)) return fail(SWEPT_EINVAL, "swept_create: alpha must be finite and positive");
     if (problem == SWEPT_EULER && !(isfinite(gamma) && gamma > 1.0)) return fail(SWEPT_EINVAL, "swept_create: gamma must be finite and > 1");
     if (p && p->max_tile_width < 0) return fail(SWEPT_EINVAL, "swept_create: max_tile_width < 0");
+    const int bc = p ? p->boundary : SWEPT_BC_PERIODIC;
+    if (bc != SWEPT_BC_PERIODIC && bc != SWEPT_BC_INSULATED) return fail(SWEPT_EINVAL, "swept_create: unknown boundary %d", bc);
+    if (bc == SWEPT_BC_INSULATED && problem != SWEPT_HEAT)
+        return fail(SWEPT_EINVAL, "swept_create: insulated ends exist for the heat problem only (the paper's KS problem is periodic, PAPER.md:66)");
 
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -105,6 +109,7 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     h->problem = problem; h->dtype = dtype;
     h->H = radius_of(problem); h->S = stages_of(problem); h->NC = ncomp_of(problem);
     h->nx = nx; h->dx = dx; h->dt = dt; h->alpha = alpha; h->gamma = gamma;
+    h->bc = bc;
     h->device = dev;
     h->kernel = SWEPT_KERNEL_WAVE;
     h->chain = 2;
@@ -170,6 +175,10 @@ static const char *width_problem(int problem, int dtype, int64_t nx, int W, int 
 
 static int check_width(const swept_ctx *h, int W, int kernel, bool set_err) {
     char buf[160];
+    if (h->bc && kernel == SWEPT_KERNEL_SMEM) {
+        if (set_err) fail(SWEPT_EINVAL, "tile_width %d: insulated ends are implemented by the WAVE kernels only", W);
+        return 0;
+    }
     const char *why = width_problem(h->problem, h->dtype, h->nx, W, kernel, h->max_smem, buf, sizeof buf);
     if (why) {
         if (set_err) fail(SWEPT_EINVAL, "tile_width %d: %s", W, why);
@@ -199,7 +208,7 @@ static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cuda
     if (h->S == 1) {
         void *a = d_u, *b = h->work;
         for (int64_t m = 0; m < nsteps; ++m) {
-            e = launch_classic_stage(h->problem, h->dtype, 1, a, a, b, h->nx, h->cb, st);
+            e = launch_classic_stage(h->problem, h->dtype, 1, a, a, b, h->nx, h->cb, h->bc, st);
             if (e != cudaSuccess) return e;
             void *t = a; a = b; b = t;
             ++*launches;
@@ -209,9 +218,9 @@ static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cuda
         }
     } else {
         for (int64_t m = 0; m < nsteps; ++m) {
-            e = launch_classic_stage(h->problem, h->dtype, 1, d_u, d_u, h->work, h->nx, h->cb, st);
+            e = launch_classic_stage(h->problem, h->dtype, 1, d_u, d_u, h->work, h->nx, h->cb, h->bc, st);
             if (e != cudaSuccess) return e;
-            e = launch_classic_stage(h->problem, h->dtype, 0, h->work, d_u, d_u, h->nx, h->cb, st);
+            e = launch_classic_stage(h->problem, h->dtype, 0, h->work, d_u, d_u, h->nx, h->cb, h->bc, st);
             if (e != cudaSuccess) return e;
             *launches += 2;
         }
@@ -339,7 +348,7 @@ static int effective_cap(const swept_ctx *h, int W);
 
 static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, int W, int64_t offset, cudaStream_t st) {
     if (kernel == SWEPT_KERNEL_SMEM) return launch_swept_smem(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, st);
-    return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, effective_cap(h, W), st);
+    return launch_swept_wave(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, h->warps_per_block, effective_cap(h, W), h->bc, st);
 }
 
 // The launch-free variant swept_run uses for width W: the option, except that with the default (2 = streaming bands) the
@@ -375,14 +384,16 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
                 }
                 break;
             case SWEPT_LAUNCH_BAND:
-                e = launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, st);
-                if (e != cudaErrorNotSupported) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
+                // bands wrap around the periodic domain; a rod with insulated ends runs on the tile-flag kernel
+                e = h->bc ? cudaErrorNotSupported
+                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, st);
+                if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
                 cudaGetLastError();
                 /* the band schedule does not fit this device / size: same half-cycles through the tile-flag kernel */
                 /* fall through */
             case SWEPT_LAUNCH_CHAIN:
                 e = launch_swept_chain(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->warps_per_block,
-                                       effective_cap(h, L.tile_width), h->sm_count, st);
+                                       effective_cap(h, L.tile_width), h->sm_count, h->bc, st);
                 h->last_sweep_launch = SWEPT_LAUNCH_CHAIN;
                 ++*launches;
                 break;
@@ -555,6 +566,7 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->sm_count = h->sm_count;
     info->max_smem_per_block = h->max_smem;
     info->last_sweep_launch = h->last_sweep_launch;
+    info->boundary = h->bc;
     info->tuned_chain = h->tuned_chain;
     info->tuned_blocks_per_sm = h->tuned_cap;
     return SWEPT_OK;

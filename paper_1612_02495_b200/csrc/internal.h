@@ -18,8 +18,9 @@ enum { MODE_UP = 0, MODE_DIAMOND = 1, MODE_DOWN = 2 };
 
 // One classic sub-timestep over all nx points (naive.cu).  odd: predictor stage of a two-stage scheme.
 // dst[i] = stage(win_src[i-H..i+H], base[i]); base may alias dst.
+// bc: SWEPT_BC_PERIODIC | SWEPT_BC_INSULATED (heat only: ghost value = adjacent interior value).
 cudaError_t launch_classic_stage(int problem, int dtype, int odd, const void *win_src, const void *base, void *dst,
-                                 int64_t nx, const ConstBlock &cb, cudaStream_t st);
+                                 int64_t nx, const ConstBlock &cb, int bc, cudaStream_t st);
 
 // Paper-style shared-memory swept kernels (swept_smem.cu): one block per tile of W points.
 // mode: MODE_UP | MODE_DIAMOND | MODE_DOWN; offset: tile-grid shift (0 or W/2).
@@ -30,11 +31,11 @@ cudaError_t swept_smem_prepare(int problem, int dtype, size_t max_bytes);
 
 // Register-resident wavefront swept kernels (swept_wave.cu): one warp per tile of W points.
 cudaError_t launch_swept_wave(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
-                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, cudaStream_t st);
+                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, int bc, cudaStream_t st);
 // Launch-free sweep: ONE launch runs q half-cycles (1 upright + (q-1) diamond + 1 closing phase), tiles ordered by per-tile
 // flags in `sync` (8 + 4*nx/W bytes, zeroed by the launch helper).
 cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
-                               int warps_per_block, int blocks_per_sm, int sm_count, cudaStream_t st);
+                               int warps_per_block, int blocks_per_sm, int sm_count, int bc, cudaStream_t st);
 // Streaming band kernel (swept_band.cuh): ONE launch runs q half-cycles with every band's columns resident in registers /
 // shared memory; `sync` = prog[nx/W] counters (zeroed by the helper).  cudaErrorNotSupported if the schedule does not fit
 // the device (the caller then uses launch_swept_chain).

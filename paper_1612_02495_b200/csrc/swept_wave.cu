@@ -5,9 +5,9 @@ namespace swept {
 
 #define DECL(prob)                                                                                                              \
     cudaError_t launch_swept_wave_##prob(int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,              \
-                                         const ConstBlock &cb, int wpb, size_t smem_floor, cudaStream_t st);                    \
+                                         const ConstBlock &cb, int wpb, size_t smem_floor, int bc, cudaStream_t st);            \
     cudaError_t launch_swept_chain_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                \
-                                          const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count, cudaStream_t st);    \
+                                          const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count, int bc, cudaStream_t st); \
     cudaError_t swept_wave_prepare_##prob(int dtype, int max_smem);                                                             \
     cudaError_t launch_swept_band_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                 \
                                          const ConstBlock &cb, int sm_count, int max_smem, cudaStream_t st);                    \
@@ -28,19 +28,19 @@ size_t smem_floor_for_cap(int cap) {
 }
 
 cudaError_t launch_swept_wave(int problem, int dtype, int mode, void *u, void *w, int64_t nx, int W, int64_t offset,
-                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, cudaStream_t st) {
+                              const ConstBlock &cb, int warps_per_block, int blocks_per_sm, int bc, cudaStream_t st) {
     const size_t floor = smem_floor_for_cap(blocks_per_sm);
-    if (problem == SWEPT_HEAT) return launch_swept_wave_heat(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
-    if (problem == SWEPT_KS) return launch_swept_wave_ks(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
-    return launch_swept_wave_euler(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, st);
+    if (problem == SWEPT_HEAT) return launch_swept_wave_heat(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, bc, st);
+    if (problem == SWEPT_KS) return launch_swept_wave_ks(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, bc, st);
+    return launch_swept_wave_euler(dtype, mode, u, w, nx, W, offset, cb, warps_per_block, floor, bc, st);
 }
 
 cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
-                               int warps_per_block, int blocks_per_sm, int sm_count, cudaStream_t st) {
+                               int warps_per_block, int blocks_per_sm, int sm_count, int bc, cudaStream_t st) {
     const size_t floor = smem_floor_for_cap(blocks_per_sm);
-    if (problem == SWEPT_HEAT) return launch_swept_chain_heat(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, st);
-    if (problem == SWEPT_KS) return launch_swept_chain_ks(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, st);
-    return launch_swept_chain_euler(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, st);
+    if (problem == SWEPT_HEAT) return launch_swept_chain_heat(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, bc, st);
+    if (problem == SWEPT_KS) return launch_swept_chain_ks(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, bc, st);
+    return launch_swept_chain_euler(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, bc, st);
 }
 
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,

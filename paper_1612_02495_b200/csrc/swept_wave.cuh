@@ -26,6 +26,17 @@
 
 namespace swept {
 
+// Global index of tile-local position g (which may lie up to W/2 + h outside [0, nx)).  Periodic: `& (nx-1)`.
+// Insulated ends (INS; the paper's heat problem, Eq. 9, reading G7 of DESIGN.md: the ghost
+// value is the adjacent interior value, T_0 = T_1): a tile that straddles an end of the rod -- the paper's "node split
+// across the spatial boundary" -- reads the mirror image -1-g / 2nx-1-g, computes the whole (symmetric)
+// diamond and stores only the positions inside the rod.
+template <bool INS> __device__ __forceinline__ int64_t dom_map(int64_t g, int64_t nx) {
+    if (!INS) return g & (nx - 1);
+    return g < 0 ? -1 - g : (g >= nx ? 2 * nx - 1 - g : g);
+}
+template <bool INS> __device__ __forceinline__ bool dom_in(int64_t g, int64_t nx) { return !INS || (g >= 0 && g < nx); }
+
 template <class T> __device__ __forceinline__ T shfl_up1(T v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
 // Staircase loads/stores.  CG = true (chained persistent kernel): cache at L2 only, because another SM may have
@@ -35,14 +46,13 @@ template <bool CG, class T> __device__ __forceinline__ void st_stair(T *p, T v) 
 
 // One tile (one warp): g0 = global index of the tile's first point (before the periodic wrap), io = the warp's
 // shared-memory row buffer of NC*W values.
-template <class P, int PW, int MODE, bool CG>
+template <class P, int PW, int MODE, bool CG, bool INS = false>
 __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real *w, const int64_t nx, const int64_t g0,
                                           typename P::real *io, const typename P::Consts &c, const int lane) {
     using T = typename P::real;
     constexpr int H = P::H, NC = P::NC, D = 2 * H;
     constexpr int W = 32 * PW, NJ = W / D, NP = PW / D, L = W / D, CTR = W / 2;
     static_assert(PW % D == 0, "points per lane must be a multiple of 2H");
-    const int64_t mask = nx - 1;
 
     // X[k][0..D) = copy of lane l-1's last D columns, X[k][D + q] = own column q
     T X[NC][D + PW];
@@ -51,14 +61,14 @@ __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real 
 #pragma unroll
         for (int k = 0; k < NC; ++k)
 #pragma unroll
-            for (int q = 0; q < PW; ++q) X[k][D + q] = ld_stair<CG>(u + (int64_t)k * nx + ((g0 + lane * PW + q) & mask));
+            for (int q = 0; q < PW; ++q) X[k][D + q] = ld_stair<CG>(u + (int64_t)k * nx + dom_map<INS>(g0 + lane * PW + q, nx));
     } else {
         // column i = 2H m + r starts from tier m of the right neighbour triangle's left edge: R_{m&1}[c + H m + r]
 #pragma unroll
         for (int q = 0; q < PW; ++q) {
             const int m = lane * NP + q / D, r = q % D;
             const T *src = (m & 1) ? w : u;
-            const int64_t g = (g0 + CTR + H * m + r) & mask;
+            const int64_t g = dom_map<INS>(g0 + CTR + H * m + r, nx);
 #pragma unroll
             for (int k = 0; k < NC; ++k) X[k][D + q] = ld_stair<CG>(src + (int64_t)k * nx + g);
         }
@@ -66,7 +76,7 @@ __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real 
         for (int j = lane; j < W; j += 32) {
             const int m = j / D, rho = j % D;
             const T *src = (m & 1) ? w : u;
-            const int64_t g = (g0 + CTR - H * m - rho - 1) & mask;
+            const int64_t g = dom_map<INS>(g0 + CTR - H * m - rho - 1, nx);
 #pragma unroll
             for (int k = 0; k < NC; ++k) io[k * W + j] = ld_stair<CG>(src + (int64_t)k * nx + g);
         }
@@ -162,31 +172,36 @@ __device__ __forceinline__ void wave_tile(typename P::real *u, typename P::real 
 #pragma unroll
         for (int k = 0; k < NC; ++k)
 #pragma unroll
-            for (int q = 0; q < PW; ++q) st_stair<CG>(u + (int64_t)k * nx + ((g0 + lane * PW + q) & mask), X[k][D + q]);
+            for (int q = 0; q < PW; ++q)
+                if (dom_in<INS>(g0 + lane * PW + q, nx)) st_stair<CG>(u + (int64_t)k * nx + dom_map<INS>(g0 + lane * PW + q, nx), X[k][D + q]);
     } else {
         // final column state: column i = 2H m + r holds tier L+m at x = H m + r  -> R_{m&1}[H m + r]
 #pragma unroll
         for (int q = 0; q < PW; ++q) {
             const int m = lane * NP + q / D, r = q % D;
             T *dst = (m & 1) ? w : u;
-            const int64_t g = (g0 + H * m + r) & mask;
+            const int64_t g = dom_map<INS>(g0 + H * m + r, nx);
+            if (dom_in<INS>(g0 + H * m + r, nx))
 #pragma unroll
-            for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, X[k][D + q]);
+                for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, X[k][D + q]);
         }
         __syncwarp();
         // lane 31's row outputs: row j = 2H m + rho holds tier L+m at x = W-1-H m-rho -> R_{m&1}[W - 1 - H m - rho]
         for (int j = lane; j < W; j += 32) {
             const int m = j / D, rho = j % D;
             T *dst = (m & 1) ? w : u;
-            const int64_t g = (g0 + W - 1 - H * m - rho) & mask;
+            const int64_t g = dom_map<INS>(g0 + W - 1 - H * m - rho, nx);
+            if (dom_in<INS>(g0 + W - 1 - H * m - rho, nx))
 #pragma unroll
-            for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, io[k * W + j]);
+                for (int k = 0; k < NC; ++k) st_stair<CG>(dst + (int64_t)k * nx + g, io[k * W + j]);
         }
     }
 }
 
 // One launch per phase (SWEPT_OPT_CHAIN = 0): stream order between the launches is the only synchronisation.
-template <class P, int PW, int MODE>
+// INS (insulated ends): a shifted launch (offset = W/2) has ntiles + 1 tiles, tile j on [jW - W/2, jW + W/2); tiles 0 and
+// ntiles straddle the ends of the rod (see dom_map).
+template <class P, int PW, int MODE, bool INS = false>
 __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, typename P::real *w, int64_t nx, int64_t offset,
                                                           int ntiles, typename P::Consts c) {
     using T = typename P::real;
@@ -196,7 +211,8 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
     const int tile = (int)blockIdx.x * (int)(blockDim.x >> 5) + warp;
     if (tile >= ntiles) return;                      // whole warps only
     T *io = reinterpret_cast<T *>(smem_raw) + (size_t)warp * P::NC * W;   // io[k*W + j]: row feed in, right edge out
-    wave_tile<P, PW, MODE, false>(u, w, nx, (int64_t)tile * W + offset, io, c, lane);
+    const int64_t g0 = (INS && offset != 0) ? (int64_t)tile * W - W / 2 : (int64_t)tile * W + offset;
+    wave_tile<P, PW, MODE, false, INS>(u, w, nx, g0, io, c, lane);
 }
 
 // ---- launch-free sweep (SWEPT_OPT_CHAIN = 1, default) ----------------------------
@@ -262,19 +278,81 @@ __global__ void __launch_bounds__((chain_max_threads<P, PW>()), (chain_min_block
     }
 }
 
+// Tile-flag kernel for insulated ends.  Even phases have ntiles tiles on [tW, (t+1)W), odd phases ntiles + 1 tiles on
+// [jW - W/2, jW + W/2); odd tile j stitches even tiles j-1 and j (where they exist), even tile t stitches odd tiles t and t+1.
+// doneE[t] / doneO[j] = 1 + the last phase of that parity the slot completed.  Items are numbered phase-major (an even
+// phase and the odd phase after it form a group of 2 ntiles + 1 items), so the smallest id in flight never waits.
+template <class P, int PW>
+__global__ void __launch_bounds__(256) swept_chain_ins_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
+                                                               unsigned long long *counter, unsigned *doneE, unsigned *doneO, typename P::Consts c) {
+    using T = typename P::real;
+    constexpr int W = 32 * PW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    T *io = reinterpret_cast<T *>(smem_raw) + (size_t)warp * P::NC * W;
+    const unsigned long long group = 2ull * (unsigned long long)ntiles + 1ull;
+    const unsigned long long total = (unsigned long long)(q + 1) * (unsigned long long)ntiles + (unsigned long long)((q + 1) / 2);
+    for (;;) {
+        unsigned long long id = 0;
+        if (lane == 0) id = atomicAdd(counter, 1ull);
+        id = __shfl_sync(0xffffffffu, id, 0);
+        if (id >= total) break;
+        const unsigned long long pair = id / group;
+        const int rem = (int)(id - pair * group);
+        const bool odd = rem >= ntiles;
+        const int p = 2 * (int)pair + (odd ? 1 : 0), t = odd ? rem - ntiles : rem;
+        if (p > 0) {
+            if (lane < 2) {
+                const unsigned *flag = nullptr;
+                if (odd) {
+                    const int s = t - 1 + lane;                  // even tiles t-1 and t
+                    if (s >= 0 && s < ntiles) flag = doneE + s;
+                } else {
+                    flag = doneO + t + lane;                     // odd tiles t and t+1
+                }
+                if (flag) {
+                    unsigned ns = 20;
+                    while (ld_acquire_gpu(flag) < (unsigned)p) {
+                        __nanosleep(ns);
+                        if (ns < 640) ns *= 2;
+                    }
+                }
+            }
+            __syncwarp();
+        }
+        const int64_t g0 = odd ? (int64_t)t * W - W / 2 : (int64_t)t * W;
+        if (p == 0) wave_tile<P, PW, MODE_UP, true, true>(u, w, nx, g0, io, c, lane);
+        else if (p == q) wave_tile<P, PW, MODE_DOWN, true, true>(u, w, nx, g0, io, c, lane);
+        else wave_tile<P, PW, MODE_DIAMOND, true, true>(u, w, nx, g0, io, c, lane);
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) st_release_gpu((odd ? doneO : doneE) + t, (unsigned)(p + 1));
+    }
+}
+
 // ---- host side, instantiated per problem in swept_wave_<problem>.cu -------------------------------------------
 template <class P, int PW>
 cudaError_t wave_launch_pw(int mode, void *u, void *w, int64_t nx, int64_t offset, const ConstBlock &cb, int wpb, size_t smem_floor,
-                           cudaStream_t st) {
+                           int bc, cudaStream_t st) {
     using T = typename P::real;
     constexpr int W = 32 * PW;
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
-    const int ntiles = (int)(nx / W);
+    const int ntiles = (int)(nx / W) + ((bc && offset != 0) ? 1 : 0);
     if (wpb > 8) wpb = 8;
     if (wpb > ntiles) wpb = ntiles;
     const unsigned blocks = (unsigned)((ntiles + wpb - 1) / wpb);
     size_t smem = (size_t)wpb * P::NC * W * sizeof(T);
     if (smem < smem_floor) smem = smem_floor;
+    if (bc) {
+        if constexpr (P::INSULATED_OK) {
+            if (mode == MODE_UP) swept_wave_kernel<P, PW, MODE_UP, true><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
+            else if (mode == MODE_DIAMOND) swept_wave_kernel<P, PW, MODE_DIAMOND, true><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
+            else swept_wave_kernel<P, PW, MODE_DOWN, true><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
+            return cudaGetLastError();
+        } else {
+            return cudaErrorNotSupported;
+        }
+    }
     if (mode == MODE_UP) swept_wave_kernel<P, PW, MODE_UP><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
     else if (mode == MODE_DIAMOND) swept_wave_kernel<P, PW, MODE_DIAMOND><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
     else swept_wave_kernel<P, PW, MODE_DOWN><<<blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, offset, ntiles, c);
@@ -284,11 +362,34 @@ cudaError_t wave_launch_pw(int mode, void *u, void *w, int64_t nx, int64_t offse
 // Chain launch: grid = min(warps needed, resident warps) / wpb blocks; `sync` = counter (8 bytes) + done[ntiles] (zeroed here).
 template <class P, int PW>
 cudaError_t wave_chain_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count,
-                          cudaStream_t st) {
+                          int bc, cudaStream_t st) {
     using T = typename P::real;
     constexpr int W = 32 * PW;
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
     const int ntiles = (int)(nx / W);
+    if (bc) {
+        // insulated ends: sync = counter (8 bytes) + doneE[ntiles] + doneO[ntiles + 1]
+        if constexpr (P::INSULATED_OK) {
+            if (wpb > 8) wpb = 8;
+            while (wpb > 1 && (int64_t)wpb * sm_count > ntiles) wpb >>= 1;
+            size_t smem = (size_t)wpb * P::NC * W * sizeof(T);
+            if (smem < smem_floor) smem = smem_floor;
+            int per_sm = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, swept_chain_ins_kernel<P, PW>, wpb * 32, smem);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+            int64_t blocks = (ntiles + 1 + wpb - 1) / wpb;
+            if (blocks > (int64_t)per_sm * sm_count) blocks = (int64_t)per_sm * sm_count;
+            e = cudaMemsetAsync(sync, 0, 8 + sizeof(unsigned) * (size_t)(2 * ntiles + 1), st);
+            if (e != cudaSuccess) return e;
+            unsigned *doneE = (unsigned *)((char *)sync + 8);
+            swept_chain_ins_kernel<P, PW><<<(unsigned)blocks, wpb * 32, smem, st>>>((T *)u, (T *)w, nx, ntiles, (int)q, (unsigned long long *)sync, doneE,
+                                                                                    doneE + ntiles, c);
+            return cudaGetLastError();
+        } else {
+            return cudaErrorNotSupported;
+        }
+    }
     if (wpb > chain_max_threads<P, PW>() / 32) wpb = chain_max_threads<P, PW>() / 32;
     while (wpb > 1 && (int64_t)wpb * sm_count > ntiles) wpb >>= 1;   // few tiles: spread the warps over the SMs
     size_t smem = (size_t)wpb * P::NC * W * sizeof(T);
@@ -313,7 +414,14 @@ template <class P, int PW> cudaError_t wave_prepare_pw(int max_smem) {
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DIAMOND>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DOWN>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    if constexpr (P::INSULATED_OK) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(swept_chain_ins_kernel<P, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_UP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DIAMOND, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(swept_wave_kernel<P, PW, MODE_DOWN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    }
+    return e;
 }
 
 }  // namespace swept

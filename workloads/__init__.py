@@ -99,6 +99,15 @@ def heat_noise(nx: int, seed: int = SEED_NOISE) -> Workload:
     return Workload(HEAT, nx, dx, dt, u0[None, :], name="heat-noise")
 
 
+def heat_rod(nx: int, seed: int = SEED_NOISE) -> Workload:
+    """The paper's heat problem: a rod with an initial temperature gradient and insulated ends -- a linear ramp
+    3 -> 0 from the left end to the right end plus grid-scale U[-1,1] noise, so that every step changes every value and the
+    two ends differ (a periodic ring would leak across the seam).  Used with boundary = insulated."""
+    dx, dt = heat_grid(nx)
+    u0 = 3.0 * (1.0 - (np.arange(nx) + 0.5) / nx) + np.random.default_rng(seed).uniform(-1.0, 1.0, nx)
+    return Workload(HEAT, nx, dx, dt, u0[None, :], name="heat-rod")
+
+
 # ----------------------------------------------------------------------------------------------
 # Kuramoto-Sivashinsky (configs 3, 5): dx = pi/4 for every nx (reading K1), dt = 0.005
 # ----------------------------------------------------------------------------------------------
