@@ -247,3 +247,68 @@ def test_band_layout_rejects_bad_arguments():
             sw.band_layout(*args)
     with pytest.raises(sw.SweptError):
         sw.band_owner(sw.band_layout(8, 4, 2), 8)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# insulated ends (SWEPT_BC_INSULATED): the split boundary node as two mirrored tiles, in the model
+# ---------------------------------------------------------------------------------------------------------------
+class RodModel(Model):
+    """The same tile model on a rod whose ghost values are the adjacent interior values: index map g -> -1-g / 2nx-1-g at every
+    load, stores only inside the rod, and one extra tile on every shifted launch (tiles on [jW - W/2, jW + W/2), j = 0..nx/W)."""
+
+    def idx(self, g):
+        return -1 - g if g < 0 else (2 * self.nx - 1 - g if g >= self.nx else g)
+
+    def naive(self, nsteps):
+        a = self.R[0].copy()
+        nx, h = self.nx, self.h
+        for _ in range(nsteps):
+            a = np.array([self.point([a[self.idx(i + k)] for k in range(-h, h + 1)], None, True) for i in range(nx)], dtype=object)
+        return a
+
+    def tile(self, mode, W, g0):
+        h = self.h
+        L, c = W // (2 * h), W // 2
+        row = [{x: self.R[0][self.idx(g0 + x)] for x in range(W)}, {}]
+        if mode != "up":
+            row[1] = {x: self.R[1][self.idx(g0 + x)] for x in range(-h, W + h)}
+        spans = []
+        if mode != "up":
+            spans += [(t, c - h * t, c + h * t) for t in range(1, L + 1)]
+        if mode != "down":
+            spans += [(t, h * t, W - h * t) for t in range(1, L)]
+        for t, lo, hi in spans:
+            src, dst = row[(t - 1) & 1], row[t & 1]
+            dst.update({x: self.point([src[x + k] for k in range(-h, h + 1)], row[0].get(x), bool(t & 1)) for x in range(lo, hi)})
+        return row
+
+    def launch(self, mode, W, offset):
+        nx, h = self.nx, self.h
+        starts = [t * W for t in range(nx // W)] if offset == 0 else [j * W - W // 2 for j in range(nx // W + 1)]
+        rows = [self.tile(mode, W, g0) for g0 in starts]
+        for g0, row in zip(starts, rows):
+            for x in range(W):
+                if 0 <= g0 + x < nx:
+                    self.R[0][g0 + x] = row[0][x]
+            if mode != "down":
+                for x in range(h, W - h):
+                    if 0 <= g0 + x < nx:
+                        self.R[1][g0 + x] = row[1][x]
+
+    def classic(self, nsteps):
+        self.R[0] = self.naive(nsteps)
+
+
+@pytest.mark.parametrize("chain", [0, 1], ids=["per-launch", "chain"])
+@pytest.mark.parametrize("nx,W,nsteps", [(64, 16, 8 * 3), (64, 16, 8 * 4 + 7), (32, 32, 16 * 3 + 5), (64, 8, 3), (48 * 0 + 128, 32, 16 * 5 + 9)])
+def test_plan_on_the_rod_model_equals_naive_stepping_with_mirrored_ghosts(nx, W, nsteps, chain):
+    """Heat-like symmetric 3-point integer stencil: the launch plan executed with two mirrored boundary tiles per shifted launch
+    reproduces naive stepping of the rod exactly (odd and even half-cycle counts, remainders, a single tile)."""
+    rng = np.random.default_rng(2495)
+    u0 = [int(v) for v in rng.integers(-5, 6, nx)]
+    plan = sw.plan(sw.HEAT, nx, nsteps, W, kernel=sw.KERNEL_SMEM, chain=chain)
+    m = RodModel(nx, 1, 1, u0)
+    m.run_plan(plan)
+    ref = RodModel(nx, 1, 1, u0).naive(nsteps)
+    assert list(m.R[0]) == list(ref)
+    assert list(ref) != list(Model(nx, 1, 1, u0).naive(nsteps))        # and the rod is not the ring
