@@ -219,8 +219,15 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
             for (int rho = 0; rho < D; ++rho) keep[sr][kk][rho] = X[kk][PW + (D - 1 - rho)];
 
     for (int K0 = 0; K0 < lt_end + 31; K0 += 32) {
-        // ---- chunk boundary (warp-uniform).  (1) flush the row outputs lane 31 produced for local times [K0-64, K0-32)
+        // ---- chunk boundary (warp-uniform).  Lane 0 first issues the acquire load of the left band's counter for the chunk it is
+        // about to fetch, so that its round trip to L2 overlaps the flush below; (1) flush the row outputs lane 31 produced for
+        // local times [K0-64, K0-32); (2) fetch the row feed of lane 0 for local times [K0, K0+32).
         __syncwarp();
+        const int sf = K0 / NJI, pf = sf / k, mf = sf - pf * k;
+        const bool fetch = K0 < lt_end && pf > 0;
+        const int bandf = first + mf * stride, left = bandf == 0 ? ntiles - 1 : bandf - 1;
+        unsigned seen = 0;
+        if (fetch && lane == 0) seen = ld_acquire_gpu(prog + left);
         const int lt0 = K0 - 64;
         if (lt0 >= 0 && lt0 < lt_end) {
             const int s = lt0 / NJI, p = s / k, m = s - p * k;
@@ -239,26 +246,24 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
                             __stcg(dst + (int64_t)kk * nx + g, outr[((kk * 64 + ((lt0 + lane) & 63)) * SR + sr) * D + rho]);
                     }
                 }
-                __threadfence();
+                // the warp barrier orders every lane's stores before lane 0's release (cumulative at gpu scope)
                 __syncwarp();
                 if (lane == 0) st_release_gpu(prog + band, (unsigned)(p * NCH + (lt0 & (NJI - 1)) / 32 + 1));
             }
         }
-        // (2) fetch the row feed of lane 0 for local times [K0, K0+32)
         if (K0 < lt_end) {
-            const int s = K0 / NJI, p = s / k, m = s - p * k;
-            if (p > 0) {
-                const int band = first + m * stride, left = band == 0 ? ntiles - 1 : band - 1;
-                const unsigned need = (unsigned)((p - 1) * NCH + (K0 & (NJI - 1)) / 32 + 1);
+            if (fetch) {
+                const unsigned need = (unsigned)((pf - 1) * NCH + (K0 & (NJI - 1)) / 32 + 1);
                 if (lane == 0) {
                     unsigned ns = 20;
-                    while (ld_acquire_gpu(prog + left) < need) {
+                    while (seen < need) {
                         __nanosleep(ns);
                         if (ns < 320) ns *= 2;
+                        seen = ld_acquire_gpu(prog + left);
                     }
                 }
                 __syncwarp();
-                const int64_t g0 = g0_of(band, p);
+                const int64_t g0 = g0_of(bandf, pf);
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr) {
                     const int J = SR * ((K0 & (NJI - 1)) + lane) + sr;         // row j = J D + rho is fed from tier J of the left tile's right edge
