@@ -32,8 +32,12 @@ namespace swept {
 // SR = super-rows a lane advances per iteration.  SR = 2 runs two consecutive super-rows one point apart (point n of the
 // first with point n-1 of the second: they are independent), which doubles the independent FP chains per warp -- heat has
 // only D = 2 rows to interleave and its DADD -> DFMA chain per point leaves the FP64 pipe idle at 4 warps per
-// sub-partition -- and halves the per-iteration overhead (shuffles, ring accesses, loop control) per update.
-template <class P, int PW> constexpr int band_sr() { return (P::H == 1 && PW >= 8) ? 2 : 1; }
+// sub-partition -- and halves the per-iteration overhead (shuffles, ring accesses, loop control) per update.  W = 512 runs
+// four: it is the width mid-size grids (2^17..2^20 points) pick, where a few warps per SM must each fill more of the pipe
+// (SR = 4 needs NJ / 4 >= 64 iterations per tile, so W = 256 stays at two and W = 1024 has no registers left for it).
+template <class P, int PW> constexpr int band_sr() {
+    return (P::H == 1 && (PW == 16 || (PW == 32 && sizeof(typename P::real) == 4))) ? 4 : ((P::H == 1 && PW >= 8) ? 2 : 1);
+}
 
 template <class P, int PW> struct BandGeom {
     using T = typename P::real;
@@ -52,6 +56,8 @@ template <class P, int PW> struct BandGeom {
 // Block size bound per instantiation: the column state alone is NC (D + PW) values per lane, so the number of warps an SM
 // can hold is set by registers; the bound tells ptxas how many registers it may use (65536 / threads).
 template <class P, int PW> constexpr int band_max_threads() {
+    // (measured: heat fp64 W = 512 with four super-rows per iteration is faster at 20 warps x 96 registers with an 80-byte
+    // spill than at 16 warps x 128 registers without one, so SR does not enter the estimate)
     const int est = P::NC * (2 * P::H + PW) * (int)(sizeof(typename P::real) / 4) + (P::GROUPED ? 110 : 56 + 16 * (P::H - 1));
     int warps = 65536 / (32 * est);
     warps = warps >= 4 ? (warps & ~3) : (warps < 1 ? 1 : warps);
