@@ -235,10 +235,12 @@ __device__ __forceinline__ void st_release_gpu(unsigned *p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// Launch bounds of the tile-flag kernel: Euler fp64 at 8 points per lane fits 170 registers, which lets a third block of
-// 4 warps onto an SM (the Euler kernels are bound by resident warps); everything else keeps 256 x 1.
-template <class P, int PW> constexpr int chain_max_threads() { return (P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8) ? 128 : 256; }
-template <class P, int PW> constexpr int chain_min_blocks() { return (P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8) ? 3 : 1; }
+// Launch bounds of the tile-flag kernel: the Euler kernels are bound by resident warps, so the narrow
+// Euler tiles are compiled for 4 blocks of 4 warps per SM (128 registers, a 200-byte spill for fp64 at 8 points per lane:
+// 29.5 GPts*steps/s at 2 blocks, 36.2 at 3, 37.2 at 4); everything else keeps 256 threads x 1 block.
+template <class P, int PW> constexpr bool chain_tight() { return P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8; }   // Euler fp64, W <= 256 (fp32 W = 512 is slower that way)
+template <class P, int PW> constexpr int chain_max_threads() { return chain_tight<P, PW>() ? 128 : 256; }
+template <class P, int PW> constexpr int chain_min_blocks() { return chain_tight<P, PW>() ? 4 : 1; }
 
 template <class P, int PW>
 __global__ void __launch_bounds__((chain_max_threads<P, PW>()), (chain_min_blocks<P, PW>())) swept_chain_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,

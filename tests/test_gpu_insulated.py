@@ -100,3 +100,26 @@ def test_insulated_ends_are_heat_only_and_need_the_wave_kernels():
         assert not s.tile_width_ok(128)
         s.set_option(sw.OPT_KERNEL, sw.KERNEL_WAVE)
         assert s.tile_width_ok(128)
+
+
+def test_full_size_rod_in_the_bench_configuration():
+    """nx = 2^22, the config's 50 000 timesteps, tuned width (what `bench.py --boundary insulated` times): swept = classic bit for
+    bit, and the left end (where the mirror matters) against the oracle on a window that the far side cannot reach: values at
+    x < M - nsteps of an M-point rod depend only on the first M points."""
+    import torch
+    nx, nsteps, M, V = 1 << 22, 50_000, 1 << 16, 4096
+    w = _rod(nx)
+    u0 = w.initial(np.float64)
+    with solver_for(w, np.float64, boundary=sw.BC_INSULATED) as s:
+        W = s.tune(to_dev(u0))
+        us, un = to_dev(u0), to_dev(u0)
+        s.swept_run(us, nsteps, 0)
+        s.naive_run(un, nsteps)
+        torch.cuda.synchronize()
+        got, naive = us.cpu().numpy(), un.cpu().numpy()
+    assert_bits_equal(got, naive, f"rod, full size, W={W}")
+    ref = oracle.heat_insulated(u0[0, :M].copy(), nsteps, w.alpha, w.dx, w.dt)
+    assert M - nsteps >= V
+    assert_bits_equal(got[0, :V], ref[:V], "left end of the rod vs the insulated oracle")
+    ref = oracle.heat_insulated(u0[0, nx - M:].copy(), nsteps, w.alpha, w.dx, w.dt)
+    assert_bits_equal(got[0, nx - V:], ref[M - V:], "right end of the rod vs the insulated oracle")
