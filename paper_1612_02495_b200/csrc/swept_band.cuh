@@ -57,7 +57,12 @@ template <class P, int PW> struct BandGeom {
 
 // Block size bound per instantiation: the column state alone is NC (D + PW) values per lane, so the number of warps an SM
 // can hold is set by registers; the bound tells ptxas how many registers it may use (65536 / threads).
-template <class P, int PW> constexpr int band_max_threads() {
+// TIGHT: a second build of the Euler fp64 narrow-tile kernel for 16 warps x 128 registers (with a spill) instead of 8 x 255: the
+// Euler kernels are bound by resident warps, so the tight build wins once the grid has more bands than 8 warps per SM can own
+// (nx = 2^19, W = 256: 37 -> 44.6 GPts*steps/s) and loses below that (2^18: 36.6 -> 32.3).
+template <class P, int PW> constexpr bool band_has_tight() { return P::GROUPED && sizeof(typename P::real) == 8 && PW <= 8; }
+
+template <class P, int PW, bool TIGHT = false> constexpr int band_max_threads() {
     // (measured: heat fp64 W = 512 with four super-rows per iteration is faster at 20 warps x 96 registers with an 80-byte
     // spill than at 16 warps x 128 registers without one, so SR does not enter the estimate)
     const int est = P::NC * (2 * P::H + PW) * (int)(sizeof(typename P::real) / 4) + (P::GROUPED ? 110 : 56 + 16 * (P::H - 1));
@@ -65,6 +70,7 @@ template <class P, int PW> constexpr int band_max_threads() {
     warps = warps >= 4 ? (warps & ~3) : (warps < 1 ? 1 : warps);
     // KS fp64 at 32 points per lane spills at the 170 registers 12 warps leave; 8 warps with up to 255 registers run faster
     if (P::H == 2 && !P::GROUPED && sizeof(typename P::real) == 8 && PW == 32) warps = 8;
+    if (TIGHT) warps = 16;
     return 32 * (warps > 32 ? 32 : warps);
 }
 
@@ -140,8 +146,8 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
     }
 }
 
-template <class P, int PW>
-__global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
+template <class P, int PW, bool TIGHT = false>
+__global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
                                                              BandGrid grid, unsigned *prog, typename P::Consts c) {
     using T = typename P::real;
     using Gm = BandGeom<P, PW>;
@@ -413,7 +419,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW>())) swept_band_kernel
 // Size the grid: one block per SM, as many warps as the kernel's registers allow (all must be resident), bands dealt
 // round-robin over the SM sub-partitions.  Returns false if the launch-free band schedule does not fit (too few
 // bands to spread over two warps, or the parked bands exceed shared memory): the caller falls back to swept_chain_kernel.
-template <class P, int PW>
+template <class P, int PW, bool TIGHT = false>
 bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *smem_bytes) {
     using Gm = BandGeom<P, PW>;
     using T = typename P::real;
@@ -424,12 +430,12 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
     if (ntiles64 < 2 || ntiles64 > (1 << 24)) return false;
     const int ntiles = (int)ntiles64;
     cudaFuncAttributes fa;
-    if (cudaFuncGetAttributes(&fa, swept_band_kernel<P, PW>) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (cudaFuncGetAttributes(&fa, swept_band_kernel<P, PW, TIGHT>) != cudaSuccess) { cudaGetLastError(); return false; }
     int regs = fa.numRegs < 16 ? 16 : fa.numRegs;
     regs = (regs + 7) & ~7;                                       // allocation granularity: 8 registers per thread
     int wmax = 65536 / (regs * 32);
     if (wmax > 32) wmax = 32;
-    if (wmax > band_max_threads<P, PW>() / 32) wmax = band_max_threads<P, PW>() / 32;
+    if (wmax > band_max_threads<P, PW, TIGHT>() / 32) wmax = band_max_threads<P, PW, TIGHT>() / 32;
     static const int cand[] = {32, 28, 24, 20, 16, 12, 8, 4, 2, 1};
     int wneed = 32;                                               // smallest block that gives every band its own warp
     for (int wpb : cand)
@@ -441,7 +447,7 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
         const size_t smem = (size_t)wpb * Gm::warp_values(g.kmax) * sizeof(T);
         if (smem > (size_t)max_smem) continue;
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, swept_band_kernel<P, PW>, wpb * 32, smem) != cudaSuccess) { cudaGetLastError(); continue; }
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, swept_band_kernel<P, PW, TIGHT>, wpb * 32, smem) != cudaSuccess) { cudaGetLastError(); continue; }
         if (per_sm < 1) continue;
         *out = g;
         *smem_bytes = smem;
@@ -451,13 +457,19 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
 }
 
 // `sync` = prog[ntiles] (zeroed here).  Returns cudaErrorNotSupported when the band schedule does not fit.
-template <class P, int PW>
+template <class P, int PW, bool TIGHT = false>
 cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, cudaStream_t st) {
     using T = typename P::real;
     using Gm = BandGeom<P, PW>;
+    if constexpr (!TIGHT && band_has_tight<P, PW>()) {
+        // more bands than the roomy build has warps, and no more than the tight build has (one band per warp: its spills make
+        // the band swaps of k > 1 slower than the roomy build's)
+        if (nx / Gm::W > (int64_t)sm_count * (band_max_threads<P, PW, false>() / 32) && nx / Gm::W <= (int64_t)sm_count * (band_max_threads<P, PW, true>() / 32))
+            return wave_band_pw<P, PW, true>(u, w, nx, q, sync, cb, sm_count, max_smem, st);
+    }
     BandGrid g;
     size_t smem = 0;
-    if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW>(nx, sm_count, max_smem, &g, &smem)) return cudaErrorNotSupported;
+    if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, &g, &smem)) return cudaErrorNotSupported;
     if ((int64_t)(q + 1) * g.kmax * Gm::NJI >= ((int64_t)1 << 31) - 64) return cudaErrorNotSupported;   // the kernel's local time is an int
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
     const int ntiles = (int)(nx / Gm::W);
@@ -470,10 +482,14 @@ cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, co
     unsigned *pr = (unsigned *)sync;
     typename P::Consts cc = c;
     void *args[] = {&up, &wp, &nx, &nt, &qi, &g, &pr, &cc};
-    return cudaLaunchCooperativeKernel((const void *)swept_band_kernel<P, PW>, dim3((unsigned)g.nblocks), dim3((unsigned)(g.wpb * 32)), args, smem, st);
+    return cudaLaunchCooperativeKernel((const void *)swept_band_kernel<P, PW, TIGHT>, dim3((unsigned)g.nblocks), dim3((unsigned)(g.wpb * 32)), args, smem, st);
 }
 
 template <class P, int PW> cudaError_t band_prepare_pw(int max_smem) {
+    if constexpr (band_has_tight<P, PW>()) {
+        cudaError_t e = cudaFuncSetAttribute(swept_band_kernel<P, PW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+        if (e != cudaSuccess) return e;
+    }
     return cudaFuncSetAttribute(swept_band_kernel<P, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
 }
 
