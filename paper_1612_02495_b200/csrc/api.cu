@@ -386,7 +386,7 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
             case SWEPT_LAUNCH_BAND:
                 // bands wrap around the periodic domain; a rod with insulated ends runs on the tile-flag kernel
                 e = h->bc ? cudaErrorNotSupported
-                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, st);
+                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, 4 * effective_cap(h, L.tile_width), st);
                 if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
                 cudaGetLastError();
                 /* the band schedule does not fit this device / size: same half-cycles through the tile-flag kernel */
@@ -461,10 +461,10 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
         // default option (streaming bands): also time the tile-flag kernel, which wins where few warps fit an SM (Euler)
         for (int mode = saved_chain; mode >= (saved_chain == 2 && wave ? 1 : saved_chain) && e == cudaSuccess; --mode) {
             h->chain = mode;
-            // resident warps per SM: with no cap given, the register-resident kernels (other than the band kernel, which sizes
-            // its own grid) are also tried at 4, 3 and 2 blocks of 4 warps per SM -- fp32 and KS run faster below full occupancy
+            // resident warps per SM: with no cap given, the register-resident kernels are also tried at 4, 3 and 2 blocks of 4
+            // warps per SM (the band kernel: 16, 12, 8 warps in its one block) -- fp32 and KS run faster below full occupancy
             static const int caps_auto[] = {0, 4, 3, 2};
-            const int ncaps = (blocks_per_sm_cap == 0 && wave && mode != 2) ? 4 : 1;
+            const int ncaps = (blocks_per_sm_cap == 0 && wave) ? (mode == 2 ? 2 : 4) : 1;   // band: none and 16 warps only (measured: fewer never wins)
             for (int ci = 0; ci < ncaps && e == cudaSuccess; ++ci) {
                 const int cap = ncaps == 1 ? blocks_per_sm_cap : caps_auto[ci];
                 h->blocks_per_sm = cap;

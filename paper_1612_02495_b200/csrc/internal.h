@@ -38,9 +38,9 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
                                int warps_per_block, int blocks_per_sm, int sm_count, int bc, cudaStream_t st);
 // Streaming band kernel (swept_band.cuh): ONE launch runs q half-cycles with every band's columns resident in registers /
 // shared memory; `sync` = prog[nx/W] counters (zeroed by the helper).  cudaErrorNotSupported if the schedule does not fit
-// the device (the caller then uses launch_swept_chain).
+// the device (the caller then uses launch_swept_chain).  max_warps > 0 caps the resident warps per SM.
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
-                              int sm_count, int max_smem, cudaStream_t st);
+                              int sm_count, int max_smem, int max_warps, cudaStream_t st);
 int swept_wave_supports(int problem, int dtype, int W);
 cudaError_t swept_wave_prepare(int problem, int dtype);
 

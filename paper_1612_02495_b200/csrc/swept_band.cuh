@@ -420,7 +420,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
 // round-robin over the SM sub-partitions.  Returns false if the launch-free band schedule does not fit (too few
 // bands to spread over two warps, or the parked bands exceed shared memory): the caller falls back to swept_chain_kernel.
 template <class P, int PW, bool TIGHT = false>
-bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *smem_bytes) {
+bool band_grid(int64_t nx, int sm_count, int max_smem, int max_warps, BandGrid *out, size_t *smem_bytes) {
     using Gm = BandGeom<P, PW>;
     using T = typename P::real;
     const int64_t ntiles64 = nx / Gm::W;
@@ -436,6 +436,7 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
     int wmax = 65536 / (regs * 32);
     if (wmax > 32) wmax = 32;
     if (wmax > band_max_threads<P, PW, TIGHT>() / 32) wmax = band_max_threads<P, PW, TIGHT>() / 32;
+    if (max_warps > 0 && wmax > max_warps) wmax = max_warps;    // SWEPT_OPT_BLOCKS_PER_SM x 4 warps: fewer resident warps on request
     static const int cand[] = {32, 28, 24, 20, 16, 12, 8, 4, 2, 1};
     int wneed = 32;                                               // smallest block that gives every band its own warp
     for (int wpb : cand)
@@ -458,18 +459,19 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, BandGrid *out, size_t *sm
 
 // `sync` = prog[ntiles] (zeroed here).  Returns cudaErrorNotSupported when the band schedule does not fit.
 template <class P, int PW, bool TIGHT = false>
-cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, cudaStream_t st) {
+cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, int max_warps,
+                         cudaStream_t st) {
     using T = typename P::real;
     using Gm = BandGeom<P, PW>;
     if constexpr (!TIGHT && band_has_tight<P, PW>()) {
         // more bands than the roomy build has warps, and no more than the tight build has (one band per warp: its spills make
         // the band swaps of k > 1 slower than the roomy build's)
         if (nx / Gm::W > (int64_t)sm_count * (band_max_threads<P, PW, false>() / 32) && nx / Gm::W <= (int64_t)sm_count * (band_max_threads<P, PW, true>() / 32))
-            return wave_band_pw<P, PW, true>(u, w, nx, q, sync, cb, sm_count, max_smem, st);
+            return wave_band_pw<P, PW, true>(u, w, nx, q, sync, cb, sm_count, max_smem, max_warps, st);
     }
     BandGrid g;
     size_t smem = 0;
-    if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, &g, &smem)) return cudaErrorNotSupported;
+    if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, max_warps, &g, &smem)) return cudaErrorNotSupported;
     if ((int64_t)(q + 1) * g.kmax * Gm::NJI >= ((int64_t)1 << 31) - 64) return cudaErrorNotSupported;   // the kernel's local time is an int
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
     const int ntiles = (int)(nx / Gm::W);
