@@ -305,6 +305,11 @@ BAND_CASES = [
     (wl.EULER, np.float64, 1 << 13, 256, 7),
     (wl.EULER, np.float32, 1 << 20, 256, 3),        # 4096 bands on few resident warps
     (wl.EULER, np.float64, 1 << 18, 512, 2),
+    (wl.HEAT, np.float32, 1 << 22, 512, 5),         # four super-rows per iteration, 8192 bands: 3 per warp, swaps in the steady loop
+    (wl.HEAT, np.float64, 1 << 21, 512, 3),         # four super-rows per iteration, 2 bands per warp
+    (wl.KS, np.float32, 1 << 22, 512, 3),           # two super-rows per iteration (KS), 8192 bands
+    (wl.KS, np.float64, 1 << 20, 512, 7),           # two super-rows per iteration, one band per warp
+    (wl.EULER, np.float64, 1 << 19, 256, 3),        # the 16-warp build of the Euler fp64 band kernel
 ]
 
 
