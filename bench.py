@@ -78,6 +78,14 @@ def parse():
     return ap.parse_args()
 
 
+def workload_name(args, w) -> str:
+    """config.workload: the same string on both arms (ours and --impl reference)."""
+    if args.problem == "heat":
+        return (f"BASELINE.json configs[1]: {w.name}, FTCS {args.boundary} r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
+                f"{w.nsteps} timesteps per step")
+    return f"{w.name} nx={w.nx} {w.nsteps} timesteps per step"
+
+
 def workload(args) -> wl.Workload:
     w = wl.heat_rod(args.nx) if args.boundary == "insulated" else wl.make(args.problem, args.nx, "config")
     if args.boundary == "insulated":
@@ -201,7 +209,7 @@ def run_reference(args):
         "impl": "reference", "metric": "grid-point updates/sec", "value": val, "unit": "GPts*steps/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-        "config": {"workload": f"{w.name} nx={w.nx} {args.dtype}; CPU oracle (plain C, OpenMP) on host cores", "nx": w.nx,
+        "config": {"workload": workload_name(args, w), "arm": "CPU oracle (plain C, OpenMP) on the host cores, a bounded sample per step", "nx": w.nx,
                    "nsteps_per_step": n},
         "cpu_baseline": {"value": val, "unit": "GPts*steps/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": "GPts*steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -547,8 +555,7 @@ def main():
         "warmup": max(args.warmup, 3), "ms_per_step": t_dev_max / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {
-            "workload": f"BASELINE.json configs[1]: {w.name}, FTCS {args.boundary} r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
-                        f"{w.nsteps} timesteps per step" if args.problem == "heat" else f"{w.name} nx={w.nx} {w.nsteps} timesteps per step",
+            "workload": workload_name(args, w),
             "nx": w.nx, "nsteps_per_step": w.nsteps, "boundary": args.boundary, "tile_width": W, "kernel": (("band" if band else "chain") if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
