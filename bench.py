@@ -81,7 +81,7 @@ def parse():
 def workload_name(args, w) -> str:
     """config.workload: the same string on both arms (ours and --impl reference)."""
     if args.problem == "heat":
-        return (f"BASELINE.json configs[1]: {w.name}, FTCS {args.boundary} r=0.25, nx=2^{int(np.log2(w.nx))} (largest of the sweep), "
+        return (f"BASELINE.json configs[1]: {w.name}, FTCS {args.boundary} r=0.25, nx=2^{int(np.log2(w.nx))}{' (largest of the sweep)' if w.nx == 1 << 22 else ''}, "
                 f"{w.nsteps} timesteps per step")
     return f"{w.name} nx={w.nx} {w.nsteps} timesteps per step"
 
