@@ -312,3 +312,69 @@ def test_plan_on_the_rod_model_equals_naive_stepping_with_mirrored_ghosts(nx, W,
     ref = RodModel(nx, 1, 1, u0).naive(nsteps)
     assert list(m.R[0]) == list(ref)
     assert list(ref) != list(Model(nx, 1, 1, u0).naive(nsteps))        # and the rod is not the ring
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# streaming-band schedule: a model of the chunk / counter protocol of swept_band.cuh on the C ABI's band assignment
+# ---------------------------------------------------------------------------------------------------------------
+def _simulate_band_schedule(ntiles, sms, wpb, q, NJI):
+    """Every warp runs its tiles phase-major; local time advances in chunks of 32 iterations.  At a chunk boundary K0 a warp
+    (1) flushes the output chunk of local times [K0-64, K0-32) -- prog[band] = p NCH + c + 1 -- and (2) may enter the chunk only
+    if the left band has flushed chunk c of phase p-1.  Returns (finished, rounds): finished is False on a cycle of waits."""
+    NCH = NJI // 32
+    lay = sw.band_layout(ntiles, sms, wpb)
+    lists = {}
+    for band in range(ntiles):
+        b, w, i = sw.band_owner(lay, band)
+        lists.setdefault((b, w), {})[i] = band
+    warps = [[l[i] for i in range(len(l))] for l in lists.values()]
+    prog = [0] * ntiles
+    K0 = [0] * len(warps)                       # boundary each warp stands at
+    end = [len(bands) * (q + 1) * NJI + 31 for bands in warps]
+    flushed = [-1] * len(warps)                 # last boundary whose flush ran
+    rounds = 0
+    while any(k0 < e for k0, e in zip(K0, end)):
+        moved = False
+        rounds += 1
+        for wi, bands in enumerate(warps):
+            k = len(bands)
+            while K0[wi] < end[wi]:
+                kb = K0[wi]
+                if flushed[wi] < kb:                                   # (1) flush, once per boundary, before any waiting
+                    lt0 = kb - 64
+                    if 0 <= lt0 < k * (q + 1) * NJI:
+                        s = lt0 // NJI
+                        p, m = divmod(s, k)
+                        if p < q:
+                            prog[bands[m]] = p * NCH + (lt0 % NJI) // 32 + 1
+                    flushed[wi] = kb
+                    moved = True
+                if kb < k * (q + 1) * NJI:                             # (2) fetch: may block
+                    s = kb // NJI
+                    p, m = divmod(s, k)
+                    if p > 0:
+                        left = (bands[m] - 1) % ntiles
+                        if prog[left] < (p - 1) * NCH + (kb % NJI) // 32 + 1:
+                            break
+                K0[wi] = kb + 32
+                moved = True
+        if not moved:
+            return False, rounds
+    # every band flushed all q phases' output chunks
+    assert all(pr == q * NCH for pr in prog), prog[:8]
+    return True, rounds
+
+
+@pytest.mark.parametrize("ntiles,sms,wpb", [(2, 148, 1), (8, 148, 1), (64, 4, 4), (256, 16, 8), (1024, 148, 8), (500, 7, 12), (96, 2, 16)])
+@pytest.mark.parametrize("NJI", [64, 128, 512])
+def test_band_schedule_never_deadlocks_with_two_or_more_chunks_per_tile(ntiles, sms, wpb, NJI):
+    done, _ = _simulate_band_schedule(ntiles, sms, wpb, q=5, NJI=NJI)
+    assert done
+
+
+def test_band_schedule_with_one_chunk_per_tile_is_a_cycle_of_waits():
+    """NJI = 32 (heat W = 64, KS / Euler W = 128): at the start of phase p lane 0 needs the chunk its left neighbour flushes only
+    32 iterations after ITS phase-p start; with every band in lockstep nobody can move -- the hang observed on the GPU, and the
+    reason those widths run on the tile-flag kernel (band_grid refuses NCH < 2)."""
+    done, _ = _simulate_band_schedule(64, 148, 1, q=3, NJI=32)
+    assert not done
