@@ -179,7 +179,17 @@ def oracle_rate(w: wl.Workload, dtype, budget_s: float = 15.0, insulated: bool =
     t0 = time.perf_counter()
     oracle.run(w.problem, u0, n, **kw)
     dt = time.perf_counter() - t0
-    return w.nx * n / dt, n, dt, oracle.num_threads()
+    # the same oracle on ONE thread (state both), about 3 s
+    cores = oracle.num_threads()
+    oracle.set_num_threads(1)
+    try:
+        n1 = int(max(2, min(n, 3.0 / max(t8 / 8 * cores, 1e-9))))      # one thread is at most `cores` times slower per step
+        t0 = time.perf_counter()
+        oracle.run(w.problem, u0, n1, **kw)
+        rate1 = w.nx * n1 / (time.perf_counter() - t0)
+    finally:
+        oracle.set_num_threads(cores)
+    return w.nx * n / dt, n, dt, cores, rate1
 
 
 def run_reference(args):
@@ -546,8 +556,8 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline:
-        rate, n, el, cores = oracle_rate(w, np_dtype, insulated=args.boundary == "insulated")
-        cpu = {"value": rate / 1e9, "unit": "GPts*steps/s", "cores": cores, "kind": "oracle",
+        rate, n, el, cores, rate1 = oracle_rate(w, np_dtype, insulated=args.boundary == "insulated")
+        cpu = {"value": rate / 1e9, "unit": "GPts*steps/s", "cores": cores, "kind": "oracle", "value_1_thread": rate1 / 1e9,
                "sample": f"{n} of {w.nsteps} timesteps at nx={w.nx} ({el:.1f} s)"}
 
     out = {
