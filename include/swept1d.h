@@ -21,6 +21,8 @@
  *     available from swept_last_error() (thread-local).  Nothing is printed, nothing aborts.
  *     Numerical blow-up is not an error: values become Inf/NaN exactly as the classic path's would.
  *   - No CPU fallback exists: without a CUDA device every compute call fails with SWEPT_ECUDA.
+ *   - A handle owns device scratch (workspace, flags, cached graphs): use it from one host thread and one stream at a
+ *     time; different handles are independent and may run concurrently on different streams.
  */
 #ifndef SWEPT1D_H
 #define SWEPT1D_H
@@ -62,7 +64,8 @@ enum {
     SWEPT_OPT_KERNEL = 0,         /* SWEPT_KERNEL_*                                              */
     SWEPT_OPT_NAIVE_GRAPH = 1,    /* 1: naive_run replays a CUDA graph of its launches (default 0:
                                      plain launches = the paper's classic program)               */
-    SWEPT_OPT_BLOCKS_PER_SM = 2,  /* cap on resident blocks per SM for the swept kernels, 0 = none */
+    SWEPT_OPT_BLOCKS_PER_SM = 2,  /* cap on resident blocks per SM for the swept kernels (the band kernel, which runs one
+                                     block per SM, caps its warps at 4 x this), 0 = none / the tuner's choice        */
     SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
     SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
     SWEPT_OPT_CHAIN = 5           /* WAVE kernels, launch-free sweep (beyond the paper; removes PAPER.md:232's launch / wave
