@@ -42,13 +42,17 @@ FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP-pipe instructions of one point 
 
 def traffic_of(args, w, W, chain):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel's launch, from the committed `ncu --set full`
-    capture of this very configuration (profiles/traffic.json names the report it was read from); None if there is none."""
+    capture of this very configuration (profiles/traffic.csv names the report it was read from); None if there is none."""
     try:
-        tab = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        import csv
         key = f"{args.problem}_{args.dtype}_nx{w.nx}_W{W}_{chain if chain else args.kernel}_nsteps{w.nsteps}"
-        return tab.get(key, {}).get("dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "traffic.csv"), newline="") as f:
+            for row in csv.DictReader(f):
+                if row["key"] == key:
+                    return int(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def parse():
