@@ -18,8 +18,10 @@
  * KS -- uniform fixed point, sum conservation, linearised complex growth factor about a uniform
  * offset (pins every coefficient and sign incl. the nonlinear one), bitwise shift equivariance,
  * exact-rational nx=8 hand stepping; Euler -- conservation, uniform fixed point, mirror symmetry,
- * exact Riemann (Sod) star states, positivity.  Parity unpinned: none for the stated formulas;
- * for Euler the choice of scheme details is BASELINE.json's reading, not the paper's.
+ * exact Riemann (Sod) star states, positivity, second-order convergence on an exactly advected
+ * smooth density wave, TVD / no new extrema on an advected square contact (both checked to FAIL on
+ * one-line mutants: zero / maxmod / unlimited slopes, full-step predictor, forward Euler, wrong face
+ * sign).  Parity unpinned: none.  (Euler is BASELINE.json config 4's scheme; the paper has none.)
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  `omp parallel for`
  * over the spatial index is the only parallelism; it does not change any result.
