@@ -40,19 +40,34 @@ FP_INSTR_PER_STAGE_UPDATE = {  # thread-level FP-pipe instructions of one point 
 }
 
 
+def kernel_sources_hash() -> str:
+    """sha256 (first 16 hex digits) over the CUDA sources of the library: ties a stored ncu figure to the kernels it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1612_02495_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode())
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def traffic_of(args, w, W, chain):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel's launch, from the committed `ncu --set full`
-    capture of this very configuration (profiles/traffic.csv names the report it was read from); None if there is none."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel's launch, where it comes from): read from the
+    committed `ncu --set full` capture of this very configuration (profiles/traffic.csv names the report and the hash of the
+    kernel sources it was captured from).  (None, why) if there is no capture, or if the kernel sources changed since."""
     try:
         import csv
         key = f"{args.problem}_{args.dtype}_nx{w.nx}_W{W}_{chain if chain else args.kernel}_nsteps{w.nsteps}"
         with open(os.path.join(ROOT, "profiles", "traffic.csv"), newline="") as f:
             for row in csv.DictReader(f):
                 if row["key"] == key:
-                    return int(row["dram_bytes_per_launch"])
-    except Exception:
-        pass
-    return None
+                    if row.get("kernel_sources_sha16", "") != kernel_sources_hash():
+                        return None, f"stale: {row['report']} was captured from kernel sources {row.get('kernel_sources_sha16', '?')}, now {kernel_sources_hash()}"
+                    return int(row["dram_bytes_per_launch"]), f"{row['report']} (kernel sources {row['kernel_sources_sha16']})"
+    except Exception as e:
+        return None, f"profiles/traffic.csv unreadable: {e}"
+    return None, "no ncu --set full capture of this configuration under profiles/"
 
 
 def parse():
@@ -72,9 +87,10 @@ def parse():
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--stress", action="store_true", help="BASELINE.json configs[4]: heat, KS, Euler x fp32, fp64 at nx = 2^22, 100 000 timesteps, "
                     "every tile width 32..2048 x kernel x resident-blocks cap 1..4 (written to gpurun_out/stress.json / stress.md)")
-    ap.add_argument("--variants", default="", help="--sweep: comma list of band,chain,wave,smem (default all)")
-    ap.add_argument("--chain", type=int, default=2, choices=[0, 1, 2],
-                    help="launch-free sweep: 2 = streaming bands (default), 1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
+    ap.add_argument("--variants", default="", help="--sweep: comma list of ring,band,chain,wave,smem (default all)")
+    ap.add_argument("--chain", type=int, default=3, choices=[0, 1, 2, 3],
+                    help="launch-free sweep: 3 = ring kernel (default: bands + communication warp, remainder inside the launch), 2 = streaming bands, "
+                         "1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
     ap.add_argument("--no-chain", action="store_true", help="same as --chain 0")
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="SWEPT_OPT_BLOCKS_PER_SM for the per-tile kernels (0 = none / tuned)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -276,7 +292,7 @@ def run_sweep(args):
             t = timed(lambda: s.naive_run(u, ns_naive))
             row["naive_graph"] = nx * ns_naive / t / 1e9
             # chain = launch-free sweep (one persistent launch); wave / smem = one launch per half-cycle, plain or CUDA graph
-            for kname, kid, chain, graphs in (("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0,)), ("wave", sw.KERNEL_WAVE, 0, (0, 1)),
+            for kname, kid, chain, graphs in (("ring", sw.KERNEL_WAVE, 3, (0,)), ("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0,)), ("wave", sw.KERNEL_WAVE, 0, (0, 1)),
                                               ("smem", sw.KERNEL_SMEM, 0, (0, 1))):
                 if args.variants and kname not in args.variants.split(","):
                     continue
@@ -289,6 +305,8 @@ def run_sweep(args):
                         s.set_option(sw.OPT_SWEPT_GRAPH, graph)
                         u.copy_(u0)
                         t = timed(lambda: s.swept_run(u, w.nsteps, W), reps=3 if nx <= (1 << 20) else 2)
+                        if kname in ("ring", "band") and sw.LAUNCH_NAMES.get(s.info()["last_sweep_launch"]) != kname:
+                            continue                # the schedule does not fit this (nx, W): the run fell back, it is another row
                         row["swept"][f"{kname}/W={W}/{'graph' if graph else 'plain'}"] = nx * w.nsteps / t / 1e9
         best = max(row["swept"], key=row["swept"].get)
         row["best"], row["best_value"] = best, row["swept"][best]
@@ -345,7 +363,7 @@ def run_stress(args):
                 s.set_option(sw.OPT_NAIVE_GRAPH, 1)
                 naive = nx * ns_naive / timed(lambda: s.naive_run(u, ns_naive)) / 1e9
                 res = {}
-                for kname, kid, chain, caps in (("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0, 1, 2, 3, 4)),
+                for kname, kid, chain, caps in (("ring", sw.KERNEL_WAVE, 3, (0,)), ("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0, 1, 2, 3, 4)),
                                                 ("smem", sw.KERNEL_SMEM, 0, (0, 1, 2, 3, 4))):
                     s.set_option(sw.OPT_KERNEL, kid)
                     s.set_option(sw.OPT_CHAIN, chain)
@@ -366,8 +384,8 @@ def run_stress(args):
                             e0.record(stream); s.swept_run(u, ns, W); e1.record(stream); e1.synchronize()
                             t = e0.elapsed_time(e1) * 1e-3
                             ran = sw.LAUNCH_NAMES.get(s.info()["last_sweep_launch"], "-") if kname != "smem" else "smem"
-                            if kname == "band" and ran != "band":
-                                continue            # the band schedule does not fit: this (W) is the chain row
+                            if kname in ("ring", "band") and ran != kname:
+                                continue            # the schedule does not fit: this (W) is another kernel's row
                             res[f"{kname}/W={W}/cap={cap}"] = nx * ns / t / 1e9
                 s.set_option(sw.OPT_BLOCKS_PER_SM, 0)
             best = max(res, key=res.get)
@@ -377,8 +395,8 @@ def run_stress(args):
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     with open(os.path.join(ROOT, "gpurun_out", "stress.json"), "w") as f:
         json.dump({"unit": "GPts*steps/s", "rows": rows}, f, indent=1)
-    print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: band | chain (W, cap) | smem (W, cap) |")
-    print("|---|---|---:|---:|---|---:|---|---|---|")
+    print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: ring | band | chain (W, cap) | smem (W, cap) |")
+    print("|---|---|---:|---:|---|---:|---|---|---|---|")
     for r in rows:
         def bk(k):
             c = {n: v for n, v in r["results"].items() if n.startswith(k + "/")}
@@ -387,7 +405,7 @@ def run_stress(args):
             b = max(c, key=c.get)
             return f"{c[b]:.1f} ({b.split('/', 1)[1]})"
         print(f"| {r['problem']} | {r['dtype']} | {r['classic_graph']:.1f} | {r['best_value']:.1f} | {r['best']} | {r['best_value'] / r['classic_graph']:.1f}x | "
-              f"{bk('band')} | {bk('chain')} | {bk('smem')} |")
+              f"{bk('ring')} | {bk('band')} | {bk('chain')} | {bk('smem')} |")
 
 
 def main():
@@ -433,7 +451,11 @@ def main():
     u0_host = torch.from_numpy(w.initial(np_dtype)).pin_memory()
     u = u0_host.cuda()
     stream = torch.cuda.current_stream()
+    t_tune0 = time.perf_counter()
     W = args.tile_width or s.tune(u.clone())
+    torch.cuda.synchronize()
+    tune_ms = (time.perf_counter() - t_tune0) * 1e3 if not args.tile_width else 0.0      # wall time of swept_tune (outside the timed region)
+    tune_launches = s.info()["launches_total"]
     sph = sw.steps_per_half_cycle(w.problem, W)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
@@ -490,21 +512,33 @@ def main():
         return
 
     # ---- roofline of the dominant kernel -------------------------------------------------------------------
-    # chain (default): ONE launch of swept_chain_kernel runs the step's q half-cycles = nx*L*q stage-updates; it is timed
-    # alone (nsteps = q*sph has no remainder, so the plan is that single launch + the memset of its flags).
-    # per-launch kernels (--no-chain / smem): the diamond launch, by differencing two runs of qa and qb half-cycles.
-    H, S = sw.RADIUS[w.problem], sw.STAGES[w.problem]
+    # launch-free kernels: ONE launch runs the sweep.  ring (default): the whole step -- q half-cycles and the remainder -- is that
+    # launch, nx * S * nsteps stage-updates.  band / tile flags: q half-cycles = nx * L * q stage-updates, timed alone (nsteps = q * sph
+    # has no remainder, so the plan is that single launch + the memset of its flags).
+    # per-launch kernels (--chain 0 / smem): the diamond launch, by differencing two runs of qa and qb half-cycles.
+    pinfo = sw.problem_info(w.problem)
+    H, S = pinfo["radius"], pinfo["stages"]
     L = W // (2 * H)
     chain = kernel == sw.KERNEL_WAVE and chain_opt != 0
-    if chain:
-        q = max(1, w.nsteps // sph)
-        assert [k for k, *_ in sw.plan(w.problem, w.nx, q * sph, W, dtype=sw_dtype, chain=chain_opt)] == [sw.LAUNCH_BAND if chain_opt == 2 else sw.LAUNCH_CHAIN]
+    step_kind = s.info()["last_sweep_launch"]           # what the timed steps ran on
+    q = max(1, w.nsteps // sph)
+    if chain and step_kind == sw.LAUNCH_RING:
+        assert sw.plan(w.problem, w.nx, w.nsteps, W, dtype=sw_dtype, chain=chain_opt) == [(sw.LAUNCH_RING, W, w.nsteps % sph, w.nsteps // sph)]
+        run_q = lambda: s.swept_run(u, w.nsteps, W)
+        run_q()
+        t_launch = min(timed(run_q, 1) for _ in range(3))
+        stage_updates = w.nx * S * w.nsteps
+        lname = "ring"
+        kname = f"swept_ring_kernel W={W} ({w.nsteps // sph} half-cycles + {w.nsteps % sph} remainder timesteps in one launch)"
+        hc = w.nsteps / sph
+    elif chain:
         run_q = lambda: s.swept_run(u, q * sph, W)
         run_q()
         t_launch = min(timed(run_q, 1) for _ in range(3))
         stage_updates = w.nx * L * q
-        band = s.info()["last_sweep_launch"] == sw.LAUNCH_BAND      # False: the band schedule did not fit, swept_chain_kernel ran
-        kname = f"{'swept_band_kernel' if band else 'swept_chain_kernel'} W={W} ({q} half-cycles in one launch)"
+        lname = {sw.LAUNCH_BAND: "band", sw.LAUNCH_RING: "ring"}.get(s.info()["last_sweep_launch"], "chain")
+        kname = f"swept_{lname}_kernel W={W} ({q} half-cycles in one launch)"
+        hc = q
     else:
         def half_cycles(n):
             return lambda: s.swept_run(u, n * sph, W)
@@ -515,22 +549,27 @@ def main():
         tb = min(timed(half_cycles(qb), 1) for _ in range(3))
         t_launch = (tb - ta) / (qb - qa)
         stage_updates = w.nx * L                               # per diamond launch: every point advances L tiers
-        band = False
+        lname = ""
         kname = f"swept diamond ({'wave' if kernel == sw.KERNEL_WAVE else 'smem'}) W={W}"
+        hc = 1
+    band = lname in ("band", "ring")
     fpi = FP_INSTR_PER_STAGE_UPDATE[(args.problem, args.dtype)]
-    peak = sw.measure_alu_peak(sw_dtype)["instr_per_s"]
+    peak_meas = sw.measure_alu_peak(sw_dtype)["instr_per_s"]
     nominal = 148 * (64 if args.dtype == "f64" else 128) * 1.965e9
     achieved = fpi * stage_updates / t_launch if fpi else None
+    traffic, traffic_source = traffic_of(args, w, W, lname)
     roofline = {
         "bound": "alu", "kernel": kname,
-        "achieved": achieved / 1e12 if achieved else None, "peak": peak / 1e12, "unit": "T FP-instr/s (thread-level)",
-        "frac": (achieved / peak) if achieved else None, "traffic": traffic_of(args, w, W, (("band" if band else "chain") if chain else "")),
-        "peak_source": "measured FMA-chain microbenchmark (swept_measure_alu_peak), same process",
-        "peak_nominal": nominal / 1e12, "frac_nominal": (achieved / nominal) if achieved else None,
+        "achieved": achieved / 1e12 if achieved else None, "peak": nominal / 1e12, "unit": "T FP-instr/s (thread-level)",
+        "frac": (achieved / nominal) if achieved else None,
+        "peak_source": "nominal pipe: 148 SMs x %d lanes x 1.965 GHz (DESIGN.md section 5.3; MEASURED_PEAKS.json has no plain-ALU figure)" % (64 if args.dtype == "f64" else 128),
+        "peak_measured_alu": peak_meas / 1e12, "frac_measured_alu": (achieved / peak_meas) if achieved else None,
+        "peak_measured_alu_source": "FMA-chain microbenchmark (swept_measure_alu_peak), same process, same clocks",
+        "traffic": traffic, "traffic_source": traffic_source,
         "launch_ms": t_launch * 1e3, "fp_instr_per_stage_update": fpi, "stage_updates_per_launch": stage_updates,
-        # staircase bytes: per half-cycle every tile reads and writes both edges (4 W values), the band kernel only the
+        # staircase bytes: per half-cycle every tile reads and writes both edges (4 W values), the band / ring kernels only the
         # upper-right edge (2 W values: lane 31's row outputs out, lane 0's row feed in)
-        "hbm_algorithmic_bytes_per_launch": int((2 if band else 4) * w.nx * sw.NCOMP[w.problem] * u.element_size() * (q if chain else 1)),
+        "hbm_algorithmic_bytes_per_launch": int((2 if band else 4) * w.nx * pinfo["ncomp"] * u.element_size() * hc),
     }
 
     # ---- classic path on the same workload (context: swept / classic speedup) ------------------------------
@@ -570,7 +609,10 @@ def main():
         "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {
             "workload": workload_name(args, w),
-            "nx": w.nx, "nsteps_per_step": w.nsteps, "boundary": args.boundary, "tile_width": W, "kernel": (("band" if band else "chain") if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
+            "nx": w.nx, "nsteps_per_step": w.nsteps, "boundary": args.boundary, "tile_width": W,
+            "kernel": (lname if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
+            "tile_width_source": "--tile-width" if args.tile_width else "swept_tune, before the timed region",
+            "tune_ms": tune_ms, "tune_launches": int(tune_launches),
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
         },

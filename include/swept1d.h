@@ -21,8 +21,15 @@
  *     available from swept_last_error() (thread-local).  Nothing is printed, nothing aborts.
  *     Numerical blow-up is not an error: values become Inf/NaN exactly as the classic path's would.
  *   - No CPU fallback exists: without a CUDA device every compute call fails with SWEPT_ECUDA.
- *   - A handle owns device scratch (workspace, flags, cached graphs): use it from one host thread and one stream at a
- *     time; different handles are independent and may run concurrently on different streams.
+ *   - A handle owns device scratch (workspace, flags, cached graphs) on the device that was current at swept_create; every
+ *     later call must be made with that device current (SWEPT_EINVAL otherwise).  Use a handle from one host thread at a
+ *     time.  Calls on one handle from different streams are legal: each call first makes its stream wait (on the device,
+ *     cudaStreamWaitEvent) for the handle's previous call, so they run one after the other.  Different handles are
+ *     independent and run concurrently on different streams.  (A call made inside the caller's own stream capture skips
+ *     that wait; the caller's graph must then order the handle's uses itself.)
+ *   - The launch-free kernels wait on flags other warps of the same launch publish; every such wait is bounded (seconds).
+ *     A wait that gives up makes the kernel exit, and the next call on the handle returns SWEPT_ECUDA once: the field that
+ *     launch ran on is invalid.
  */
 #ifndef SWEPT1D_H
 #define SWEPT1D_H
@@ -70,7 +77,12 @@ enum {
     SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
     SWEPT_OPT_CHAIN = 5           /* WAVE kernels, launch-free sweep (beyond the paper; removes PAPER.md:232's launch / wave
                                      costs): ONE persistent launch runs all half-cycles of a swept_run.
-                                     2 (default) = streaming bands: a warp keeps its tile's columns in registers from one
+                                     3 (default) = streaming bands with a communication warp per block: as 2, but the edge
+                                         exchange is staged by cp.async through shared-memory rings by a dedicated warp, so the
+                                         computing warps never wait on global memory, and the remainder timesteps (nsteps mod
+                                         L/S) run inside the same launch as a truncated closing cycle: swept_run is
+                                         ONE launch for any nsteps.  Falls back to 2 where the width / schedule does not fit.
+                                     2 = streaming bands: a warp keeps its tile's columns in registers from one
                                          half-cycle to the next (the upper-left edge of PAPER.md Fig. 2b never leaves the
                                          SM), only the upper-right edge travels through global memory, ordered by one
                                          progress counter per band; falls back to 1 when the schedule does not fit.
@@ -90,8 +102,12 @@ enum {
  *   DOWN     closing inverted triangles at `offset`
  *   CHAIN    `count` half-cycles (1 UP + (count-1) DIAMOND + 1 DOWN phases, offsets 0, W/2, 0, ...) in ONE launch
  *   BAND     the same in ONE launch of the streaming band kernel (SWEPT_OPT_CHAIN = 2; a handle whose device cannot hold
- *            the band schedule runs the entry as CHAIN)                                                              */
-enum { SWEPT_LAUNCH_CLASSIC = 0, SWEPT_LAUNCH_UP = 1, SWEPT_LAUNCH_DIAMOND = 2, SWEPT_LAUNCH_DOWN = 3, SWEPT_LAUNCH_CHAIN = 4, SWEPT_LAUNCH_BAND = 5 };
+ *            the band schedule runs the entry as CHAIN)
+ *   RING     `count` half-cycles AND `offset` remainder timesteps (offset < L/S; a truncated closing cycle) in ONE launch of
+ *            the ring kernel (SWEPT_OPT_CHAIN = 3): the whole swept_run.  A handle whose device cannot hold the schedule runs
+ *            the same timesteps as the plan of SWEPT_OPT_CHAIN = 2.                                                   */
+enum { SWEPT_LAUNCH_CLASSIC = 0, SWEPT_LAUNCH_UP = 1, SWEPT_LAUNCH_DIAMOND = 2, SWEPT_LAUNCH_DOWN = 3, SWEPT_LAUNCH_CHAIN = 4, SWEPT_LAUNCH_BAND = 5,
+       SWEPT_LAUNCH_RING = 6 };
 typedef struct {
     int kind;           /* SWEPT_LAUNCH_*                         */
     int tile_width;     /* W of the entry (0 for CLASSIC)         */
@@ -117,10 +133,10 @@ typedef struct {
     int sm_count;                /* multiprocessors of the device the handle lives on            */
     int max_smem_per_block;      /* opt-in shared-memory limit per block (bytes)                 */
     int last_sweep_launch;       /* SWEPT_LAUNCH_* that ran the half-cycles of the last swept_run enqueued outside a
-                                    graph (BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet        */
+                                    graph (RING, BAND, CHAIN, or DIAMOND for per-half-cycle launches); -1 = none yet  */
     int boundary;                /* SWEPT_BC_*                                                    */
-    int tuned_chain;             /* SWEPT_OPT_CHAIN value (1 | 2) swept_tune measured as faster for tuned_tile_width under
-                                    the default option 2; 0 = not tuned                                              */
+    int tuned_chain;             /* SWEPT_OPT_CHAIN value (1 | 2 | 3) swept_tune measured as fastest for tuned_tile_width
+                                    under the default option 3; 0 = not tuned                                        */
     int tuned_blocks_per_sm;     /* resident-blocks cap swept_tune measured as fastest for tuned_tile_width when called with
                                     blocks_per_sm_cap = 0 (0 = none); used while SWEPT_OPT_BLOCKS_PER_SM is 0          */
 } swept_info_t;
@@ -139,11 +155,12 @@ int swept_create(swept_handle_t *out, int problem, int64_t nx, double dx, double
  * with L = tile_width/(2h) tiers per half-cycle (L/S timesteps), q = nsteps div (L/S) half-cycles
  * are run as 1 upright triangle (Fig. 5) + (q-1) diamonds on tiles shifted by W/2 each
  * launch + 1 closing inverted triangle; the nsteps mod (L/S) remaining
- * timesteps are run first on narrower tiles / the classic kernel (the paper can only output every
- * n-th step; reading S3).  Edges are exchanged through d_u itself (even
+ * timesteps are run as a truncated closing cycle inside the same launch (ring kernel, the default) or first, on narrower
+ * tiles / the classic kernel (the other kernels; the paper can only output every n-th step; reading S3).  Edges are exchanged through d_u itself (even
  * tiers) and the handle's workspace (odd tiers) -- the paper's left/right arrays.
- * tile_width: power of two, >= 4h, <= nx, nx % tile_width == 0, L even; 0 = the tuned width (or the
- * library default if swept_tune has not run).  Result is bit-identical to naive_run.
+ * tile_width: power of two, >= 4h, <= nx, nx % tile_width == 0, L even; 0 = the tuned width, or, if swept_tune has
+ * not run, the library default: the widest legal width <= 256 of the selected kernel family -- on grids narrower than the
+ * narrowest register tile (nx < 64 h) the paper-style shared-memory kernels.  Result is bit-identical to naive_run.
  * d_u: device, [ncomp][nx], caller-owned.  Errors: SWEPT_EINVAL (NULL, nsteps < 0, illegal width
  * or a width whose tile does not fit the chosen kernel), SWEPT_ECUDA (launch error). */
 int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void *cuda_stream);
@@ -157,9 +174,10 @@ int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
 /* The launch list swept_run(h, d_u, nsteps, tile_width) enqueues for a solver of (problem, dtype, nx) with the given
  * kernel family (SWEPT_KERNEL_*) and chain option: host logic only, needs neither a handle nor a device.  Writes up
  * to `cap` entries to out (may be NULL when cap == 0) and returns the number of entries of the full plan, or a negative
- * error code (illegal width, bad arguments).  Reading S3 of DESIGN.md: with nsteps = q*(L/S) + r, the r remainder
- * timesteps come first -- one UP + DOWN pair on each narrower legal width of r's binary decomposition, then CLASSIC for
- * what is left -- followed by the q half-cycles of width tile_width. */
+ * error code (illegal width, bad arguments).  Reading S3 of DESIGN.md: with nsteps = q*(L/S) + r, chain = 3 gives the single
+ * entry RING(count = q, offset = r) where the ring kernel takes the width (at least 64 iterations per tile, two tiles); else the
+ * r remainder timesteps come first -- one UP + DOWN pair on each narrower legal width of r's binary decomposition, then CLASSIC
+ * for what is left -- followed by the q half-cycles of width tile_width. */
 int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int tile_width, int kernel, int chain,
                    swept_launch_t *out, int64_t cap);
 
@@ -177,9 +195,9 @@ int swept_band_owner(const swept_band_layout_t *layout, int band, int *block, in
 /* The paper's best-node-size sweep: time swept_run on d_u_scratch (device,
  * [ncomp][nx], contents destroyed) for every legal tile width (and kernel launch shape) up to
  * max_tile_width with at most blocks_per_sm_cap resident blocks per SM (0 = no cap), keep the
- * fastest in the handle and return it in *best_tile_width (may be NULL).  Under the default SWEPT_OPT_CHAIN = 2 each
- * width is timed with the streaming band kernel and with the tile-flag kernel, and swept_run uses the faster of the two
- * for the tuned width; with blocks_per_sm_cap = 0 the register-resident per-tile kernels are also timed at 4, 3 and 2 blocks
+ * fastest in the handle and return it in *best_tile_width (may be NULL).  Under the default SWEPT_OPT_CHAIN = 3 each
+ * width is timed with the ring kernel, the streaming band kernel and the tile-flag kernel, and swept_run uses the fastest of
+ * the three for the tuned width; with blocks_per_sm_cap = 0 the register-resident per-tile kernels are also timed at 4, 3 and 2 blocks
  * of 4 warps per SM (the paper's occupancy trade-off).  SYNCHRONISES the stream. */
 int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream);
 
@@ -190,6 +208,10 @@ int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int tile_width, 
 
 /* Set a SWEPT_OPT_* option.  SWEPT_EINVAL for unknown keys / values. */
 int swept_set_option(swept_handle_t h, int key, int value);
+
+/* Stencil radius h per sub-timestep, sub-timesteps S per timestep and fields per point of `problem` (any pointer may be
+ * NULL): a half-cycle of tile width W advances W / (2 h S) timesteps.  Host logic, no device needed. */
+int swept_problem_info(int problem, int *radius, int *stages, int *ncomp);
 
 /* Fill *info (caller-owned). */
 int swept_get_info(swept_handle_t h, swept_info_t *info);

@@ -19,21 +19,18 @@ HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
 OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN = 0, 1, 2, 3, 4, 5
-LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND = 0, 1, 2, 3, 4, 5
-LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band"}
+LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
+LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}
 BC_PERIODIC, BC_INSULATED = 0, 1
-CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS = 0, 1, 2     # values of OPT_CHAIN (include/swept1d.h); CHAIN_BANDS is the default
+CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS, CHAIN_RING = 0, 1, 2, 3     # values of OPT_CHAIN (include/swept1d.h); CHAIN_RING is the default
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
-RADIUS = {HEAT: 1, KS: 2, EULER: 2}
-STAGES = {HEAT: 1, KS: 2, EULER: 2}
-NCOMP = {HEAT: 1, KS: 1, EULER: 3}
 
 # every symbol include/swept1d.h declares
 SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
-    "swept_band_layout", "swept_band_owner",
+    "swept_band_layout", "swept_band_owner", "swept_problem_info",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -101,6 +98,7 @@ def lib() -> ctypes.CDLL:
     L.swept_plan.argtypes = [ci, ci, i64, i64, ci, ci, ci, ctypes.POINTER(_Launch), i64]
     L.swept_band_layout.argtypes = [ci, ci, ci, ctypes.POINTER(_BandLayout)]
     L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
+    L.swept_problem_info.argtypes = [ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     for name in SYMBOLS:
         getattr(L, name).restype = ci
     L.swept_plan.restype = i64
@@ -151,6 +149,9 @@ class Solver:
         self.problem, self.nx, self.dtype = int(problem), int(nx), _dtype_id(dtype)
         p = _Params(self.dtype, float(alpha), float(gamma), int(max_tile_width), int(boundary))
         _check(lib().swept_create(ctypes.byref(self._h), self.problem, self.nx, float(dx), float(dt), ctypes.byref(p)))
+        import torch
+        self.device = torch.cuda.current_device()      # swept_create binds the handle to the current device
+        self.ncomp = self.info()["ncomp"]
 
     # -- marshalling ----------------------------------------------------------------------------------------
     def _ptr(self, u) -> int:
@@ -158,8 +159,10 @@ class Solver:
         want = torch.float64 if self.dtype == F64 else torch.float32
         if not (isinstance(u, torch.Tensor) and u.is_cuda and u.is_contiguous() and u.dtype == want):
             raise SweptError(EINVAL, "u must be a contiguous CUDA tensor of the handle's dtype")
-        if u.numel() != NCOMP[self.problem] * self.nx:
-            raise SweptError(EINVAL, f"u must hold ncomp*nx = {NCOMP[self.problem] * self.nx} elements")
+        if u.device.index != self.device:
+            raise SweptError(EINVAL, f"u lives on cuda:{u.device.index} but the handle was created on cuda:{self.device}")
+        if u.numel() != self.ncomp * self.nx:
+            raise SweptError(EINVAL, f"u must hold ncomp*nx = {self.ncomp * self.nx} elements")
         return u.data_ptr()
 
     def swept_run(self, u, nsteps: int, tile_width: int = 0, stream=None) -> None:
@@ -185,7 +188,7 @@ class Solver:
             ptr, n, es = h_u.ctypes.data, h_u.size, h_u.itemsize
         else:
             raise SweptError(EINVAL, "h_u must be a contiguous CPU tensor or numpy array")
-        if n != NCOMP[self.problem] * self.nx or es != (8 if self.dtype == F64 else 4):
+        if n != self.ncomp * self.nx or es != (8 if self.dtype == F64 else 4):
             raise SweptError(EINVAL, "h_u has the wrong size or dtype")
         _check(lib().swept_run_host(self._h, ptr, int(nsteps), int(tile_width), 1 if use_swept else 0, _stream_ptr(stream)))
 
@@ -225,7 +228,7 @@ def measure_alu_peak(dtype=F64, stream=None) -> dict:
     return {"instr_per_s": ips.value, "ms": ms.value}
 
 
-def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: int = CHAIN_BANDS) -> list:
+def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: int = CHAIN_RING) -> list:
     """The launch list `swept_run` enqueues (swept_plan; host logic, no device needed): [(kind, W, offset, count), ...]."""
     buf = (_Launch * 64)()
     n = lib().swept_plan(int(problem), int(dtype), int(nx), int(nsteps), int(tile_width), int(kernel), int(chain), buf, 64)
@@ -249,6 +252,14 @@ def band_owner(layout: dict, band: int) -> tuple:
     return b.value, w.value, i.value
 
 
+def problem_info(problem: int) -> dict:
+    """Stencil radius per sub-timestep, sub-timesteps per timestep and fields per point (swept_problem_info; no device needed)."""
+    r, s, n = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(lib().swept_problem_info(int(problem), ctypes.byref(r), ctypes.byref(s), ctypes.byref(n)))
+    return {"radius": r.value, "stages": s.value, "ncomp": n.value}
+
+
 def steps_per_half_cycle(problem: int, tile_width: int) -> int:
     """L/S: full timesteps one half-cycle advances."""
-    return tile_width // (2 * RADIUS[problem] * STAGES[problem])
+    i = problem_info(problem)
+    return tile_width // (2 * i["radius"] * i["stages"])

@@ -23,12 +23,16 @@ struct swept_ctx {
     void *host_stage;      // device buffer for swept_run_host (allocated on first use)
     int device, sm_count, max_smem;
     int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
-    void *sync;            // chain kernel: work counter (8 bytes) + done[nx / 8] flags
+    void *sync_base;       // SYNC_HEADER bytes (word 0: the abort word of the bounded waits, swept_wave.cuh) + the sync area
+    void *sync;            // sync area = sync_base + SYNC_HEADER; chain kernel: work counter (8 bytes) + done[] flags; band kernel: prog[]
+    unsigned *abort_seen;  // pinned host copy of the abort word, refreshed by an async copy behind every launch-free launch
+    cudaEvent_t busy;      // recorded behind the work of every call; the next call's stream waits on it (calls on one handle
+                           // from several streams are serialised on the device instead of corrupting the shared scratch)
     int max_tile_width, tuned_tile_width, tuned_chain, tuned_cap, last_sweep_launch;   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
-    cudaGraphExec_t sgraph;  void *sgraph_u;  int64_t sgraph_steps;  int sgraph_W, sgraph_kernel, sgraph_chain;
+    cudaGraphExec_t sgraph;  void *sgraph_u;  int64_t sgraph_steps;  int sgraph_W, sgraph_kernel, sgraph_chain, sgraph_cap, sgraph_wpb;
     int64_t sgraph_launches;
 };
 
@@ -112,7 +116,7 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     h->bc = bc;
     h->device = dev;
     h->kernel = SWEPT_KERNEL_WAVE;
-    h->chain = 2;
+    h->chain = 3;
     h->last_sweep_launch = -1;
     h->warps_per_block = 4;
     h->max_tile_width = p ? p->max_tile_width : 0;
@@ -126,16 +130,26 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
         cudaGetLastError();
         return fail(e == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "swept_create: cudaMalloc workspace: %s", cudaGetErrorString(e));
     }
-    e = cudaMalloc(&h->sync, 8 + sizeof(unsigned) * (size_t)(nx / 8));
+    e = cudaMalloc(&h->sync_base, SYNC_HEADER + 8 + sizeof(unsigned) * (size_t)(nx / 8 + 2));
     if (e != cudaSuccess) {
         cudaFree(h->work);
         delete h;
         cudaGetLastError();
         return fail(e == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "swept_create: cudaMalloc flags: %s", cudaGetErrorString(e));
     }
-    e = swept_smem_prepare(problem, dtype, (size_t)h->max_smem);
+    h->sync = (char *)h->sync_base + SYNC_HEADER;
+    e = cudaMemset(h->sync_base, 0, SYNC_HEADER);
+    if (e == cudaSuccess) e = cudaHostAlloc((void **)&h->abort_seen, sizeof(unsigned), cudaHostAllocDefault);
+    if (e == cudaSuccess) { *h->abort_seen = 0; e = cudaEventCreateWithFlags(&h->busy, cudaEventDisableTiming); }
+    if (e == cudaSuccess) e = swept_smem_prepare(problem, dtype, (size_t)h->max_smem);
     if (e == cudaSuccess) e = swept_wave_prepare(problem, dtype);
-    if (e != cudaSuccess) { cudaFree(h->work); cudaFree(h->sync); delete h; return fail_cuda(e, "swept_create: kernel attribute setup"); }
+    if (e != cudaSuccess) {
+        cudaFree(h->work); cudaFree(h->sync_base);
+        if (h->abort_seen) cudaFreeHost(h->abort_seen);
+        if (h->busy) cudaEventDestroy(h->busy);
+        delete h;
+        return fail_cuda(e, "swept_create: scratch / kernel attribute setup");
+    }
     *out = h;
     return SWEPT_OK;
 }
@@ -149,7 +163,9 @@ extern "C" int swept_destroy(swept_handle_t h) {
     if (!h) return fail(SWEPT_EINVAL, "swept_destroy: NULL handle");
     drop_graphs(h);
     if (h->work) cudaFree(h->work);
-    if (h->sync) cudaFree(h->sync);
+    if (h->sync_base) cudaFree(h->sync_base);
+    if (h->abort_seen) cudaFreeHost(h->abort_seen);
+    if (h->busy) cudaEventDestroy(h->busy);
     if (h->host_stage) cudaFree(h->host_stage);
     delete h;
     return SWEPT_OK;
@@ -192,12 +208,51 @@ extern "C" int swept_tile_width_ok(swept_handle_t h, int tile_width) {
     return check_width(h, tile_width, h->kernel, true);
 }
 
-static int default_width(const swept_ctx *h) {
+// The width swept_run uses for tile_width = 0: the tuned one, else the largest legal width not above 256 (WAVE) / 512 (SMEM)
+// and nx.  Grids too small for the narrowest register tile (32 lanes x 2h points) fall back to the paper-style shared-memory
+// kernels, which take any power of two >= 4h: *kernel is the family to run.
+static int default_width(const swept_ctx *h, int *kernel) {
+    *kernel = h->kernel;
     if (h->tuned_tile_width) return h->tuned_tile_width;
-    // largest legal width not above 256 (WAVE) / 512 (SMEM) and nx
     for (int W = h->kernel == SWEPT_KERNEL_WAVE ? 256 : 512; W >= 4 * h->H; W >>= 1)
         if (check_width(h, W, h->kernel, false)) return W;
+    if (h->kernel == SWEPT_KERNEL_WAVE && !h->bc) {
+        *kernel = SWEPT_KERNEL_SMEM;
+        for (int W = 512; W >= 4 * h->H; W >>= 1)
+            if (check_width(h, W, SWEPT_KERNEL_SMEM, false)) return W;
+    }
     return 0;
+}
+
+// ---- entry / exit of every call that enqueues work on a handle ---------------------------------------------------
+// The handle's device (the kernels' shared-memory opt-ins and the scratch are per device) must be current; a wait that gave up
+// in an earlier launch-free sweep is reported once; the stream first waits for the handle's previous call (any stream).
+static int handle_enter(swept_ctx *h, cudaStream_t st, const char *who) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, who);
+    if (dev != h->device) return fail(SWEPT_EINVAL, "%s: the handle was created on device %d but device %d is current", who, h->device, dev);
+    if (*(volatile unsigned *)h->abort_seen) {
+        cudaStreamSynchronize(st);
+        *h->abort_seen = 0;
+        cudaMemset(h->sync_base, 0, SYNC_HEADER);
+        return fail(SWEPT_ECUDA, "%s: an earlier launch-free sweep on this handle gave up waiting for a tile that never completed "
+                                 "(was the handle used from two host threads at once?); the field it ran on is invalid", who);
+    }
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+    if (cs == cudaStreamCaptureStatusNone) {
+        e = cudaStreamWaitEvent(st, h->busy, 0);
+        if (e != cudaSuccess) return fail_cuda(e, who);
+    }
+    return SWEPT_OK;
+}
+static void handle_leave(swept_ctx *h, cudaStream_t st) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); return; }
+    if (cs != cudaStreamCaptureStatusNone) return;     // the caller's own capture orders its nodes
+    cudaMemcpyAsync(h->abort_seen, h->sync_base, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
+    cudaEventRecord(h->busy, st);
 }
 
 // ---- classic path (row A2) -----------------------------------------------------------------------------------
@@ -267,6 +322,7 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
     int rc = run_args_ok(h, d_u, nsteps, "naive_run");
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = handle_enter(h, st, "naive_run"))) return rc;
     int64_t launches = 0;
     if (h->naive_graph && nsteps >= 2) {
         // a graph of `chunk` timesteps (even, so heat's ping-pong ends in d_u), replayed; the rest as plain launches
@@ -287,6 +343,7 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
         cudaError_t e = enqueue_classic(h, d_u, nsteps, st, &launches);
         if (e != cudaSuccess) return fail_cuda(e, "naive_run");
     }
+    handle_leave(h, st);
     h->launches_last = launches;
     h->launches_total += launches;
     return SWEPT_OK;
@@ -299,7 +356,7 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
 // half-cycles of width W: 1 upright triangle + (q-1) diamonds on tiles shifted by W/2 each launch + 1 closing inverted
 // triangle; on a periodic domain either alignment may write out (reading S4).  With `chain` (WAVE
 // kernels) the q half-cycles are ONE launch of the flag-ordered persistent kernel.
-static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int W, int kernel, int chain, int max_smem,
+static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, int W, int kernel, int chain, int bc, int max_smem,
                           swept_launch_t *out, int64_t cap) {
     const int H = radius_of(problem), S = stages_of(problem);
     const int per = 2 * H * S;   // W / per = timesteps per half-cycle
@@ -310,7 +367,7 @@ static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, in
     };
     auto half_cycles = [&](int w, int64_t q, bool chained) {
         if (q <= 0) return;
-        if (chained) { push(chain == 2 ? SWEPT_LAUNCH_BAND : SWEPT_LAUNCH_CHAIN, w, 0, q); return; }
+        if (chained) { push(chain >= 2 ? SWEPT_LAUNCH_BAND : SWEPT_LAUNCH_CHAIN, w, 0, q); return; }
         push(SWEPT_LAUNCH_UP, w, 0, 1);
         if (q > 1) push(SWEPT_LAUNCH_DIAMOND, w, w / 2, q - 1);   // offsets W/2, 0, W/2, ...
         push(SWEPT_LAUNCH_DOWN, w, (q & 1) ? w / 2 : 0, 1);
@@ -318,6 +375,11 @@ static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, in
     const int64_t sph = W / per;
     const int64_t q = nsteps / sph;
     int64_t r = nsteps % sph;
+    // ring kernel (chain = 3): the q half-cycles AND the remainder (as a truncated closing cycle) in one launch; entry.offset = r
+    if (chain == 3 && kernel == SWEPT_KERNEL_WAVE && !bc && nsteps > 0 && swept_ring_supports(problem, W) && nx / W >= 2) {
+        push(SWEPT_LAUNCH_RING, W, r, q);
+        return n;
+    }
     char buf[160];
     for (int w = W / 2; w >= 4 * H && r > 0; w >>= 1) {
         const int64_t s = w / per;
@@ -341,7 +403,8 @@ extern "C" int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps
     char buf[160];
     const char *why = width_problem(problem, dtype, nx, tile_width, kernel, SWEPT_SMEM_LIMIT_B200, buf, sizeof buf);
     if (why) return fail(SWEPT_EINVAL, "tile_width %d: %s", tile_width, why);
-    return build_plan(problem, dtype, nx, nsteps, tile_width, kernel, chain, SWEPT_SMEM_LIMIT_B200, out, cap);
+    if (chain < 0 || chain > 3) return fail(SWEPT_EINVAL, "swept_plan: chain takes 0..3");
+    return build_plan(problem, dtype, nx, nsteps, tile_width, kernel, chain, SWEPT_BC_PERIODIC, SWEPT_SMEM_LIMIT_B200, out, cap);
 }
 
 static int effective_cap(const swept_ctx *h, int W);
@@ -354,7 +417,7 @@ static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, i
 // The launch-free variant swept_run uses for width W: the option, except that with the default (2 = streaming bands) the
 // tuner's measured choice between the band and the tile-flag kernel is honoured for the width it tuned.
 static int effective_chain(const swept_ctx *h, int W) {
-    if (h->chain == 2 && h->tuned_chain && W == h->tuned_tile_width) return h->tuned_chain;
+    if (h->chain == 3 && h->tuned_chain && W == h->tuned_tile_width) return h->tuned_chain;
     return h->chain;
 }
 
@@ -364,9 +427,10 @@ static int effective_cap(const swept_ctx *h, int W) {
     return h->blocks_per_sm;
 }
 
-static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches) {
+static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t nsteps, int W, cudaStream_t st, int64_t *launches, int chain_override = -1) {
     swept_launch_t plan[64];   // at most 3 entries per narrower width + 1 classic + 3
-    const int64_t n = build_plan(h->problem, h->dtype, h->nx, nsteps, W, kernel, effective_chain(h, W), h->max_smem, plan, 64);
+    const int chain = chain_override >= 0 ? chain_override : effective_chain(h, W);
+    const int64_t n = build_plan(h->problem, h->dtype, h->nx, nsteps, W, kernel, chain, h->bc, h->max_smem, plan, 64);
     if (n > 64) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
     for (int64_t i = 0; i < n && e == cudaSuccess; ++i) {
@@ -383,6 +447,13 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
                     ++*launches;
                 }
                 break;
+            case SWEPT_LAUNCH_RING:
+                e = launch_swept_ring(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, (int)(L.offset * h->S), h->sync, h->cb, h->sm_count, h->max_smem,
+                                      4 * effective_cap(h, L.tile_width), st);
+                if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_RING; break; }
+                cudaGetLastError();
+                // the ring schedule does not fit this device / size: the same timesteps as remainder launches + band / tile-flag kernel
+                return enqueue_swept(h, kernel, d_u, nsteps, W, st, launches, 2);
             case SWEPT_LAUNCH_BAND:
                 // bands wrap around the periodic domain; a rod with insulated ends runs on the tile-flag kernel
                 e = h->bc ? cudaErrorNotSupported
@@ -406,24 +477,28 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
 extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_width, void *cuda_stream) {
     int rc = run_args_ok(h, d_u, nsteps, "swept_run");
     if (rc) return rc;
-    int W = tile_width;
+    int W = tile_width, kernel = h->kernel;
     if (W == 0) {
-        W = default_width(h);
+        W = default_width(h, &kernel);
         if (W == 0) return fail(SWEPT_EINVAL, "swept_run: no legal tile width for nx=%lld with the selected kernel", (long long)h->nx);
     } else if (!check_width(h, W, h->kernel, true)) return SWEPT_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = handle_enter(h, st, "swept_run"))) return rc;
     int64_t launches = 0;
     if (h->swept_graph && nsteps > 0) {
-        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == h->kernel && h->sgraph_chain == effective_chain(h, W);
+        const int chain = effective_chain(h, W), cap = effective_cap(h, W);
+        const bool reuse = h->sgraph && h->sgraph_u == d_u && h->sgraph_steps == nsteps && h->sgraph_W == W && h->sgraph_kernel == kernel && h->sgraph_chain == chain &&
+                           h->sgraph_cap == cap && h->sgraph_wpb == h->warps_per_block;
         int64_t l = 0;
-        rc = run_graphed(&h->sgraph, reuse, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_swept(h, h->kernel, d_u, nsteps, W, s, n); }, "swept_run(graph)");
+        rc = run_graphed(&h->sgraph, reuse, st, &l, [&](cudaStream_t s, int64_t *n) { return enqueue_swept(h, kernel, d_u, nsteps, W, s, n); }, "swept_run(graph)");
         if (rc) return rc;
-        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = h->kernel; h->sgraph_chain = effective_chain(h, W); h->sgraph_launches = l; }
+        if (!reuse) { h->sgraph_u = d_u; h->sgraph_steps = nsteps; h->sgraph_W = W; h->sgraph_kernel = kernel; h->sgraph_chain = chain; h->sgraph_cap = cap; h->sgraph_wpb = h->warps_per_block; h->sgraph_launches = l; }
         launches = h->sgraph_launches;
     } else {
-        cudaError_t e = enqueue_swept(h, h->kernel, d_u, nsteps, W, st, &launches);
+        cudaError_t e = enqueue_swept(h, kernel, d_u, nsteps, W, st, &launches);
         if (e != cudaSuccess) return fail_cuda(e, "swept_run");
     }
+    handle_leave(h, st);
     h->launches_last = launches;
     h->launches_total += launches;
     return SWEPT_OK;
@@ -435,6 +510,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     if (rc) return rc;
     if (blocks_per_sm_cap < 0) return fail(SWEPT_EINVAL, "swept_tune: blocks_per_sm_cap < 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((rc = handle_enter(h, st, "swept_tune"))) return rc;
     const int saved_cap = h->blocks_per_sm, saved_graph = h->swept_graph;
     h->blocks_per_sm = blocks_per_sm_cap;
     h->swept_graph = 0;
@@ -458,13 +534,14 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     const bool wave = h->kernel == SWEPT_KERNEL_WAVE;
     for (int W = 4 * h->H; W <= wtop && e == cudaSuccess; W <<= 1) {
         if (!check_width(h, W, h->kernel, false)) continue;
-        // default option (streaming bands): also time the tile-flag kernel, which wins where few warps fit an SM (Euler)
-        for (int mode = saved_chain; mode >= (saved_chain == 2 && wave ? 1 : saved_chain) && e == cudaSuccess; --mode) {
+        // default option (ring kernel): also time the band kernel with in-warp exchange (one more computing warp per SM on the
+        // largest grids) and the tile-flag kernel (wins where few warps fit an SM)
+        for (int mode = saved_chain; mode >= (saved_chain == 3 && wave ? 1 : saved_chain) && e == cudaSuccess; --mode) {
             h->chain = mode;
             // resident warps per SM: with no cap given, the register-resident kernels are also tried at 4, 3 and 2 blocks of 4
             // warps per SM (the band kernel: 16, 12, 8 warps in its one block) -- fp32 and KS run faster below full occupancy
             static const int caps_auto[] = {0, 4, 3, 2};
-            const int ncaps = (blocks_per_sm_cap == 0 && wave) ? (mode == 2 ? 2 : 4) : 1;   // band: none and 16 warps only (measured: fewer never wins)
+            const int ncaps = (blocks_per_sm_cap == 0 && wave) ? (mode >= 2 ? 2 : 4) : 1;   // band / ring: none and 16 warps only (measured: fewer never wins)
             for (int ci = 0; ci < ncaps && e == cudaSuccess; ++ci) {
                 const int cap = ncaps == 1 ? blocks_per_sm_cap : caps_auto[ci];
                 h->blocks_per_sm = cap;
@@ -489,9 +566,11 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     cudaEventDestroy(e1);
     h->blocks_per_sm = saved_cap;
     h->swept_graph = saved_graph;
+    handle_leave(h, st);
     if (e != cudaSuccess) return fail_cuda(e, "swept_tune");
+    drop_graphs(h);                                      // a cached swept graph was captured with the pre-tune launch shape
     h->tuned_tile_width = best;
-    h->tuned_chain = (saved_chain == 2 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
+    h->tuned_chain = (saved_chain == 3 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
     h->tuned_cap = blocks_per_sm_cap == 0 ? best_cap : 0;
     if (best_tile_width) *best_tile_width = best;
     return SWEPT_OK;
@@ -504,6 +583,8 @@ extern "C" int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int t
     if (nsteps < 0) return fail(SWEPT_EINVAL, "swept_run_host: nsteps < 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e;
+    int rc0 = handle_enter(h, st, "swept_run_host");
+    if (rc0) return rc0;
     if (!h->host_stage) {
         e = cudaMalloc(&h->host_stage, h->field_bytes);
         if (e != cudaSuccess) { cudaGetLastError(); h->host_stage = nullptr; return fail(SWEPT_ENOMEM, "swept_run_host: cudaMalloc: %s", cudaGetErrorString(e)); }
@@ -536,7 +617,7 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
             h->swept_graph = value;
             return SWEPT_OK;
         case SWEPT_OPT_CHAIN:
-            if (value != 0 && value != 1 && value != 2) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0, 1 or 2");
+            if (value < 0 || value > 3) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0, 1, 2 or 3");
             h->chain = value;
             return SWEPT_OK;
         case SWEPT_OPT_BLOCKS_PER_SM:
@@ -591,6 +672,14 @@ extern "C" int swept_band_owner(const swept_band_layout_t *lay, int band, int *b
     g.nblocks = lay->blocks; g.wpb = lay->warps_per_block; g.SL = lay->slots_per_block; g.wps = lay->warps_per_slot;
     g.G = lay->slots; g.kmax = lay->max_bands_per_warp;
     band_owner(g, band, block, warp, index);
+    return SWEPT_OK;
+}
+
+extern "C" int swept_problem_info(int problem, int *radius, int *stages, int *ncomp) {
+    if (problem != SWEPT_HEAT && problem != SWEPT_KS && problem != SWEPT_EULER) return fail(SWEPT_EINVAL, "swept_problem_info: unknown problem %d", problem);
+    if (radius) *radius = radius_of(problem);
+    if (stages) *stages = stages_of(problem);
+    if (ncomp) *ncomp = ncomp_of(problem);
     return SWEPT_OK;
 }
 

@@ -16,6 +16,10 @@ struct ConstBlock {
 
 enum { MODE_UP = 0, MODE_DIAMOND = 1, MODE_DOWN = 2 };
 
+// Bytes in front of a handle's sync area (flags / counters of the launch-free kernels); word 0 is the abort word of the
+// bounded waits (swept_wave.cuh: spin_gives_up).  The launch helpers zero the sync area, never the header.
+constexpr int SYNC_HEADER = 16;
+
 // One classic sub-timestep over all nx points (naive.cu).  odd: predictor stage of a two-stage scheme.
 // dst[i] = stage(win_src[i-H..i+H], base[i]); base may alias dst.
 // bc: SWEPT_BC_PERIODIC | SWEPT_BC_INSULATED (heat only: ghost value = adjacent interior value).
@@ -41,6 +45,12 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
 // the device (the caller then uses launch_swept_chain).  max_warps > 0 caps the resident warps per SM.
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
                               int sm_count, int max_smem, int max_warps, cudaStream_t st);
+// Ring kernel (swept_ring.cuh): the band kernel with a communication warp per block (cp.async-staged edge exchange); ONE launch
+// runs q half-cycles plus rt remainder tiers (rt = S x remaining timesteps < L).  `sync` = prog[nx/W] counters (zeroed by the
+// helper).  cudaErrorNotSupported if the width / schedule does not fit (the caller then uses the band or the tile-flag kernel).
+cudaError_t launch_swept_ring(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,
+                              int sm_count, int max_smem, int max_warps, cudaStream_t st);
+int swept_ring_supports(int problem, int W);
 int swept_wave_supports(int problem, int dtype, int W);
 cudaError_t swept_wave_prepare(int problem, int dtype);
 

@@ -268,15 +268,18 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         if (K0 < lt_end) {
             if (fetch) {
                 const unsigned need = (unsigned)((pf - 1) * NCH + (K0 & (NJI - 1)) / 32 + 1);
+                bool dead = false;
                 if (lane == 0) {
                     unsigned ns = 20;
+                    SpinWatch polls;
                     while (seen < need) {
                         __nanosleep(ns);
                         if (ns < 320) ns *= 2;
                         seen = ld_acquire_gpu(prog + left);
+                        if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
                     }
                 }
-                __syncwarp();
+                if (__any_sync(0xffffffffu, dead)) return;    // (also the warp barrier behind lane 0's acquire)
                 const int64_t g0 = g0_of(bandf, pf);
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr) {

@@ -12,6 +12,10 @@ namespace swept {
     cudaError_t launch_swept_band_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                 \
                                          const ConstBlock &cb, int sm_count, int max_smem, int max_warps, cudaStream_t st);     \
     cudaError_t swept_band_prepare_##prob(int dtype, int max_smem);                                                             \
+    cudaError_t launch_swept_ring_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync,         \
+                                         const ConstBlock &cb, int sm_count, int max_smem, int max_warps, cudaStream_t st);     \
+    cudaError_t swept_ring_prepare_##prob(int dtype, int max_smem);                                                             \
+    int swept_ring_supports_##prob(int W);                                                                                      \
     int swept_wave_supports_##prob(int W);
 DECL(heat)
 DECL(ks)
@@ -50,6 +54,19 @@ cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t 
     return launch_swept_band_euler(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, st);
 }
 
+cudaError_t launch_swept_ring(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,
+                              int sm_count, int max_smem, int max_warps, cudaStream_t st) {
+    if (problem == SWEPT_HEAT) return launch_swept_ring_heat(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
+    if (problem == SWEPT_KS) return launch_swept_ring_ks(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
+    return launch_swept_ring_euler(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
+}
+
+int swept_ring_supports(int problem, int W) {
+    if (problem == SWEPT_HEAT) return swept_ring_supports_heat(W);
+    if (problem == SWEPT_KS) return swept_ring_supports_ks(W);
+    return swept_ring_supports_euler(W);
+}
+
 int swept_wave_supports(int problem, int dtype, int W) {
     (void)dtype;
     if (problem == SWEPT_HEAT) return swept_wave_supports_heat(W);
@@ -64,13 +81,16 @@ cudaError_t swept_wave_prepare(int problem, int dtype) {
     cudaError_t e;
     if (problem == SWEPT_HEAT) {
         if ((e = swept_wave_prepare_heat(dtype, max_smem)) != cudaSuccess) return e;
+        if ((e = swept_ring_prepare_heat(dtype, max_smem)) != cudaSuccess) return e;
         return swept_band_prepare_heat(dtype, max_smem);
     }
     if (problem == SWEPT_KS) {
         if ((e = swept_wave_prepare_ks(dtype, max_smem)) != cudaSuccess) return e;
+        if ((e = swept_ring_prepare_ks(dtype, max_smem)) != cudaSuccess) return e;
         return swept_band_prepare_ks(dtype, max_smem);
     }
     if ((e = swept_wave_prepare_euler(dtype, max_smem)) != cudaSuccess) return e;
+    if ((e = swept_ring_prepare_euler(dtype, max_smem)) != cudaSuccess) return e;
     return swept_band_prepare_euler(dtype, max_smem);
 }
 

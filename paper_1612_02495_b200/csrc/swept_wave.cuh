@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(256) swept_wave_kernel(typename P::real *u, ty
     wave_tile<P, PW, MODE, false, INS>(u, w, nx, g0, io, c, lane);
 }
 
-// ---- launch-free sweep (SWEPT_OPT_CHAIN = 1, default) ----------------------------
+// ---- launch-free sweep (SWEPT_OPT_CHAIN = 1) ----------------------------
 // ONE launch runs all q half-cycles: phase 0 = upright triangles (offset 0), phases 1..q-1 = diamonds (offset W/2, 0,
 // W/2, ...), phase q = closing inverted triangles.  Work items (phase, tile) are handed out in phase-major order by an
 // atomic counter; a warp that draws (p, t) waits until the two tiles of phase p-1 it stitches together (PAPER.md:86,
@@ -233,6 +233,27 @@ __device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned *p) {
 }
 __device__ __forceinline__ void st_release_gpu(unsigned *p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Bounded waits.  The launch-free kernels wait on flags / counters that other warps of the SAME launch publish; a flag
+// that never comes (a grid that is not fully resident, a handle misused from two host threads) would otherwise spin for ever
+// and take the GPU with it.  Every SPIN_CHECK polls a waiting warp looks at the clock and at the handle's abort word -- the 4
+// bytes SYNC_HEADER bytes before the sync area the helpers zero; after SPIN_LIMIT_NS of waiting it sets that word itself.
+// A warp that sees the word set leaves the kernel; the host reports SWEPT_ECUDA from the next call on the handle (api.cu).
+// The result of such a run is garbage.
+struct SpinWatch { unsigned polls = 0; unsigned long long t0 = 0; };
+constexpr unsigned SPIN_CHECK = 1024;
+constexpr unsigned long long SPIN_LIMIT_NS = 4000000000ull;
+__device__ __forceinline__ unsigned *abort_word_of(void *sync_area) { return reinterpret_cast<unsigned *>(reinterpret_cast<char *>(sync_area) - SYNC_HEADER); }
+__device__ __forceinline__ bool spin_gives_up(SpinWatch &sw, unsigned *abortw) {
+    if ((++sw.polls & (SPIN_CHECK - 1)) != 0) return false;
+    if (*reinterpret_cast<volatile unsigned *>(abortw) != 0) return true;
+    unsigned long long now;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+    if (sw.t0 == 0) { sw.t0 = now; return false; }
+    if (now - sw.t0 < SPIN_LIMIT_NS) return false;
+    atomicExch(abortw, 1u);
+    return true;
 }
 
 // Launch bounds of the tile-flag kernel: the Euler kernels are bound by resident warps, so the narrow
@@ -259,16 +280,19 @@ __global__ void __launch_bounds__((chain_max_threads<P, PW>()), (chain_min_block
         const int p = (int)(id / (unsigned long long)ntiles);
         const int t = (int)(id - (unsigned long long)p * (unsigned long long)ntiles);
         if (p > 0) {
+            bool dead = false;
             if (lane < 2) {
                 int slot = t;
                 if (lane == 1) slot = (p & 1) ? (t + 1 == ntiles ? 0 : t + 1) : (t == 0 ? ntiles - 1 : t - 1);
                 unsigned ns = 20;
+                    SpinWatch polls;
                 while (ld_acquire_gpu(done + slot) < (unsigned)p) {
                     __nanosleep(ns);
                     if (ns < 640) ns *= 2;
+                    if (spin_gives_up(polls, abort_word_of(counter))) { dead = true; break; }
                 }
             }
-            __syncwarp();
+            if (__any_sync(0xffffffffu, dead)) return;        // (also the warp barrier that orders the other lanes behind the acquire)
         }
         const int64_t g0 = (int64_t)t * W + ((p & 1) ? W / 2 : 0);
         if (p == 0) wave_tile<P, PW, MODE_UP, true>(u, w, nx, g0, io, c, lane);
@@ -304,6 +328,7 @@ __global__ void __launch_bounds__(256) swept_chain_ins_kernel(typename P::real *
         const bool odd = rem >= ntiles;
         const int p = 2 * (int)pair + (odd ? 1 : 0), t = odd ? rem - ntiles : rem;
         if (p > 0) {
+            bool dead = false;
             if (lane < 2) {
                 const unsigned *flag = nullptr;
                 if (odd) {
@@ -314,13 +339,15 @@ __global__ void __launch_bounds__(256) swept_chain_ins_kernel(typename P::real *
                 }
                 if (flag) {
                     unsigned ns = 20;
+                    SpinWatch polls;
                     while (ld_acquire_gpu(flag) < (unsigned)p) {
                         __nanosleep(ns);
                         if (ns < 640) ns *= 2;
+                        if (spin_gives_up(polls, abort_word_of(counter))) { dead = true; break; }
                     }
                 }
             }
-            __syncwarp();
+            if (__any_sync(0xffffffffu, dead)) return;
         }
         const int64_t g0 = odd ? (int64_t)t * W - W / 2 : (int64_t)t * W;
         if (p == 0) wave_tile<P, PW, MODE_UP, true, true>(u, w, nx, g0, io, c, lane);
@@ -361,7 +388,8 @@ cudaError_t wave_launch_pw(int mode, void *u, void *w, int64_t nx, int64_t offse
     return cudaGetLastError();
 }
 
-// Chain launch: grid = min(warps needed, resident warps) / wpb blocks; `sync` = counter (8 bytes) + done[ntiles] (zeroed here).
+// Chain launch: grid = min(warps needed, resident warps) / wpb blocks; `sync` = counter (8 bytes) + done[ntiles] (zeroed here);
+// the handle's abort word sits SYNC_HEADER bytes before it (not zeroed here).
 template <class P, int PW>
 cudaError_t wave_chain_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count,
                           int bc, cudaStream_t st) {

@@ -32,9 +32,9 @@ def run_naive(w: wl.Workload, dtype, nsteps: int, u0=None, graph: bool = False) 
 
 
 # the swept kernel variants every parity test runs: (kernel family, chain option)
-SMEM, WAVE, CHAIN, BAND = (sw.KERNEL_SMEM, 0), (sw.KERNEL_WAVE, 0), (sw.KERNEL_WAVE, 1), (sw.KERNEL_WAVE, 2)
-VARIANTS = [SMEM, WAVE, CHAIN, BAND]
-VARIANT_IDS = ["smem", "wave", "chain", "band"]
+SMEM, WAVE, CHAIN, BAND, RING = (sw.KERNEL_SMEM, 0), (sw.KERNEL_WAVE, 0), (sw.KERNEL_WAVE, 1), (sw.KERNEL_WAVE, 2), (sw.KERNEL_WAVE, 3)
+VARIANTS = [SMEM, WAVE, CHAIN, BAND, RING]
+VARIANT_IDS = ["smem", "wave", "chain", "band", "ring"]
 
 
 def _select(s: sw.Solver, kernel) -> None:

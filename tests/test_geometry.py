@@ -55,7 +55,7 @@ def test_paper_geometry_numbers():
     # a 32-point node gives four KS timesteps per (half-)cycle, "which only reduces instances of communication
     # by 1/8": one global exchange per L = 8 sub-timesteps = 4 two-stage timesteps
     assert sw.steps_per_half_cycle(sw.KS, 32) == g["ks_steps_per_cycle_n32"]
-    assert 32 // (2 * sw.RADIUS[sw.KS]) == 8
+    assert 32 // (2 * sw.problem_info(sw.KS)["radius"]) == 8
 
 
 def test_triangle_counts_sum_to_whole_tiers():
@@ -114,6 +114,44 @@ class Model:
             self.updates += hi - lo
         return row
 
+    def tile_window(self, W, g0, lo, hi):
+        """One diamond tile restricted to the tiers lo < t <= hi of its 2L - 1 (t <= L: the expanding part; the ring kernel's
+        per-phase window, swept_ring.cuh).  (0, L] is "down", (L, 2L - 1] is "up", (0, 2L - 1] the whole diamond."""
+        nx, h = self.nx, self.h
+        L, c = W // (2 * h), W // 2
+        row = [{x: self.R[0][(g0 + x) % nx] for x in range(W)}, {x: self.R[1][(g0 + x) % nx] for x in range(-h, W + h)}]
+        spans = [(t, c - h * t, c + h * t) for t in range(1, L + 1)] + [(L + t, h * t, W - h * t) for t in range(1, L)]
+        for t, a, b in spans:
+            if not (lo < t <= hi):
+                continue
+            src, dst = row[(t - 1) & 1], row[t & 1]
+            new = {x: self.point([src[x + k] for k in range(-h, h + 1)], row[0].get(x), bool(t & 1)) for x in range(a, b)}
+            dst.update(new)
+            self.updates += b - a
+        return row
+
+    def ring(self, W, q, r):
+        """SWEPT_LAUNCH_RING: q half-cycles and r remainder timesteps in one sweep.  Phase p runs the tiers (lo, hi] of every
+        diamond of its alignment: lo = L in phase 0 (the flat field is tier L of the first diamonds), hi = L + rt in phase q and
+        rt in the extra phase q + 1, rt = S r (the truncated closing cycle).  The flat result is tier rt of the phase-(q+1) tiles
+        where they reach it and tier L + rt of the phase-q tiles elsewhere: both have the parity of rt."""
+        nx, h = self.nx, self.h
+        L, rt = W // (2 * h), self.S * r
+        assert 0 <= rt < L
+        nph = q + 1 + (1 if rt else 0)
+        for p in range(nph):
+            lo = L if p == 0 else 0
+            hi = 2 * L - 1 if p < q else (L + rt if p == q else rt)
+            offset = W // 2 if p & 1 else 0
+            rows = [self.tile_window(W, t * W + offset, lo, hi) for t in range(nx // W)]
+            for t, row in enumerate(rows):
+                g0 = t * W + offset
+                for x in range(W):
+                    self.R[0][(g0 + x) % nx] = row[0][x]
+                for x in range(h, W - h):
+                    self.R[1][(g0 + x) % nx] = row[1][x]
+        self.R[0] = self.R[rt & 1].copy()
+
     def launch(self, mode, W, offset):
         nx, h = self.nx, self.h
         rows = [self.tile(mode, W, t * W + offset) for t in range(nx // W)]     # all tiles read before any writes ...
@@ -143,6 +181,8 @@ class Model:
             elif kind in (sw.LAUNCH_CHAIN, sw.LAUNCH_BAND):      # the same phases in one launch (tile flags / streaming bands)
                 for p in range(count + 1):
                     self.launch("up" if p == 0 else ("down" if p == count else "diamond"), W, W // 2 if p & 1 else 0)
+            elif kind == sw.LAUNCH_RING:
+                self.ring(W, count, offset)
             else:
                 raise AssertionError(kind)
 
@@ -162,7 +202,7 @@ CASES = [
 @pytest.mark.parametrize("chain", [0, 1, 2], ids=["per-launch", "chain", "band"])
 @pytest.mark.parametrize("problem,nx,W,nsteps", CASES)
 def test_plan_executed_on_the_model_equals_naive_stepping(problem, nx, W, nsteps, chain):
-    h, S = sw.RADIUS[problem], sw.STAGES[problem]
+    h, S = sw.problem_info(problem)["radius"], sw.problem_info(problem)["stages"]
     rng = np.random.default_rng(1612)
     u0 = [int(v) for v in rng.integers(-5, 6, nx)]
     plan = sw.plan(problem, nx, nsteps, W, kernel=sw.KERNEL_SMEM, chain=chain)
@@ -187,12 +227,47 @@ def test_plan_structure_and_launch_counts():
     assert [(k, W) for k, W, _, _ in plan] == [(sw.LAUNCH_UP, 512), (sw.LAUNCH_DOWN, 512), (sw.LAUNCH_UP, 128), (sw.LAUNCH_DOWN, 128),
                                                (sw.LAUNCH_CLASSIC, 0), (sw.LAUNCH_CHAIN, 1024)]
     assert plan[-1][3] == 97 and plan[-2][3] == 16
-    # the default (SWEPT_OPT_CHAIN = 2, streaming bands) differs only in the kind of the last entry
-    band = sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE)
+    # SWEPT_OPT_CHAIN = 2 (streaming bands) differs only in the kind of the last entry
+    band = sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE, chain=sw.CHAIN_BANDS)
     assert band[:-1] == plan[:-1] and band[-1] == (sw.LAUNCH_BAND, 1024, 0, 97)
-    # q = 0: everything classic or narrower tiles
+    # the default (SWEPT_OPT_CHAIN = 3, ring kernel): ONE launch, the 336 remainder timesteps as a truncated closing cycle
+    assert sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_RING, 1024, 336, 97)]
+    assert sw.plan(sw.KS, 4096, 3, 256, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_RING, 256, 3, 0)]           # q = 0: only the truncated cycle
+    # widths the ring kernel does not take (a tile shorter than 64 iterations; a single tile): the plan of option 2
+    assert sw.plan(sw.HEAT, 1024, 10000, 64, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_CLASSIC, 0, 0, 16), (sw.LAUNCH_BAND, 64, 0, 312)]
+    assert [k for k, *_ in sw.plan(sw.HEAT, 256, 300, 256, kernel=sw.KERNEL_WAVE)][-1] == sw.LAUNCH_BAND
+    # q = 0 without the ring kernel: everything classic or narrower tiles
     assert sw.plan(sw.KS, 4096, 3, 128, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_CLASSIC, 0, 0, 3)]
     assert sw.plan(sw.KS, 4096, 0, 128) == []
+
+
+RING_CASES = [
+    # problem, nx, W, nsteps: the truncated closing cycle on the plain-Python model (any W: the model has no 64-iteration limit)
+    (sw.HEAT, 64, 16, 8 * 3),            # no remainder: phase q closes at tier L
+    (sw.HEAT, 64, 16, 8 * 4 + 7),        # odd remainder: the flat result sits on the odd staircase row
+    (sw.HEAT, 64, 16, 8 * 3 + 2),
+    (sw.HEAT, 32, 16, 5),                # q = 0: the upright triangle truncated at tier L + 5, then tiers 1..5 of the shifted tiles
+    (sw.HEAT, 64, 32, 16 * 2 + 15),      # remainder L - 1
+    (sw.KS, 64, 16, 2 * 3 + 1),
+    (sw.KS, 64, 32, 4 * 2 + 3),
+    (sw.KS, 64, 32, 1),
+    (sw.EULER, 64, 32, 4 * 3 + 2),
+]
+
+
+@pytest.mark.parametrize("problem,nx,W,nsteps", RING_CASES)
+def test_ring_plan_with_truncated_closing_cycle_equals_naive_stepping(problem, nx, W, nsteps):
+    """The remainder inside the launch: q half-cycles + r timesteps as phases with tier windows."""
+    info = sw.problem_info(problem)
+    h, S = info["radius"], info["stages"]
+    rng = np.random.default_rng(2495)
+    u0 = [int(v) for v in rng.integers(-5, 6, nx)]
+    sph = W // (2 * h * S)
+    m = Model(nx, h, S, u0)
+    m.run_plan([(sw.LAUNCH_RING, W, nsteps % sph, nsteps // sph)])
+    ref = Model(nx, h, S, u0).naive(nsteps)
+    assert list(m.R[0]) == list(ref)
+    assert m.updates == nx * S * nsteps          # every (point, tier) exactly once
 
 
 def test_plan_rejects_illegal_widths():

@@ -51,7 +51,7 @@ def test_full_size_bench_configuration(problem, dtype, nx, kind, M):
         W = s.tune(to_dev(u0))                       # what bench.py does: tuned width, chain on (the default)
         assert s.tile_width_ok(W)
         kinds = [k for k, *_ in sw.plan(problem, nx, nsteps, W, dtype=sw.F64 if dtype == np.float64 else sw.F32)]
-        assert kinds[-1] == sw.LAUNCH_BAND               # the default: streaming bands (runs as CHAIN where they do not fit)
+        assert kinds == [sw.LAUNCH_RING]                 # the default: the whole run, remainder included, is ONE launch of the ring kernel
         us, un = to_dev(u0), to_dev(u0)
         s.swept_run(us, nsteps, 0)                   # 0 = the tuned width
         s.naive_run(un, nsteps)
@@ -91,3 +91,36 @@ def test_full_size_config5_prefix_and_width_sweep():
                 assert_bits_equal(us.cpu().numpy(), naive, f"config5 {wl.PROBLEM_NAMES[problem]} W={W}")
         idx, ref = _oracle_window(w, dtype, u0, nsteps, 0, 1 << 14)
         assert_bits_equal(naive.reshape(u0.shape)[:, idx], ref, "config5 oracle window")
+
+
+CONFIG5 = [(wl.HEAT, np.float64), (wl.HEAT, np.float32), (wl.KS, np.float64), (wl.KS, np.float32), (wl.EULER, np.float64), (wl.EULER, np.float32)]
+
+
+@pytest.mark.parametrize("problem,dtype", CONFIG5, ids=[f"{wl.PROBLEM_NAMES[p]}-{'f64' if d == np.float64 else 'f32'}" for p, d in CONFIG5])
+def test_full_size_config5_full_length(problem, dtype):
+    """Config 5 at its FULL length: nx = 2^22, 100 000 timesteps on the 16-mode series, all six
+    (problem, dtype) pairs, in the configuration the stress bench times (tuned width, default launch-free option):
+    swept == classic bit for bit over the whole field; the oracle on the window of a 1 000-step prefix."""
+    import torch
+    nx, nsteps, prefix = 1 << 22, 100_000, 1000
+    w = wl.make(problem, nx, "config5")
+    assert w.nsteps == nsteps
+    u0 = w.initial(dtype)
+    with solver_for(w, dtype) as s:
+        W = s.tune(to_dev(u0))
+        s.set_option(sw.OPT_NAIVE_GRAPH, 1)              # same kernels, same order; only the launch mechanism differs
+        us, un, up = to_dev(u0), to_dev(u0), to_dev(u0)
+        s.swept_run(us, nsteps, 0)
+        ran = s.info()["last_sweep_launch"]
+        s.naive_run(un, nsteps)
+        s.swept_run(up, prefix, 0)
+        torch.cuda.synchronize()
+        got, naive, pre = us.cpu().numpy(), un.cpu().numpy(), up.cpu().numpy()
+    assert ran in (sw.LAUNCH_RING, sw.LAUNCH_BAND, sw.LAUNCH_CHAIN)
+    assert np.all(np.isfinite(naive)) and not np.array_equal(naive, u0)
+    assert_bits_equal(got, naive, f"config5 full length swept({sw.LAUNCH_NAMES[ran]}, W={W}) vs classic")
+    for centre in (0, nx // 2 + W // 2):
+        idx, ref = _oracle_window(w, dtype, u0, prefix, centre, 1 << 14)
+        sample = pre.reshape(u0.shape)[:, idx]
+        assert rel_max(sample, ref) <= TOL[dtype]
+        assert_bits_equal(sample, ref, f"config5 prefix vs oracle window at {centre}")

@@ -10,6 +10,7 @@ import pytest
 
 import paper_1612_02495_b200 as sw
 import workloads as wl
+from gpu_util import SMEM as SMEM_V, BAND as BAND_V
 from gpu_util import (VARIANTS, VARIANT_IDS, TOL, assert_bits_equal, rel_max, run_naive, run_oracle, run_swept, solver_for, to_dev, width_ok)
 
 pytestmark = pytest.mark.gpu
@@ -331,8 +332,8 @@ def test_band_kernel_equals_classic(problem, dtype, nx, W, q):
 
 
 def test_band_falls_back_to_tile_flags_where_the_schedule_does_not_fit():
-    """One 32-iteration chunk per tile (heat W = 64) and a single band (nx = W) cannot run as streaming bands: the same
-    half-cycles run on swept_chain_kernel, with the same result."""
+    """One 32-iteration chunk per tile (heat W = 64) and a single band (nx = W) can run neither on the ring kernel nor as
+    streaming bands: the same half-cycles run on swept_chain_kernel, with the same result."""
     import torch
     for nx, W in ((1 << 12, 64), (256, 256)):
         w = _noise(wl.HEAT, nx)
@@ -349,6 +350,8 @@ def test_band_repeated_calls_two_streams_and_graph_replay():
     import torch
     w = _noise(wl.HEAT, 1 << 20)
     s1, s2 = solver_for(w, np.float64), solver_for(w, np.float64)
+    s1.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
+    s2.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
     s2.set_option(sw.OPT_SWEPT_GRAPH, 1)
     st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
     u1, u2 = to_dev(w.initial(np.float64)), to_dev(w.initial(np.float64))
@@ -369,6 +372,146 @@ def test_tuner_chooses_between_bands_and_tile_flags():
     with solver_for(w, np.float64) as s:
         W = s.tune(to_dev(w.initial(np.float64)))
         info = s.info()
-        assert info["tuned_tile_width"] == W and info["tuned_chain"] in (sw.CHAIN_TILES, sw.CHAIN_BANDS)
+        assert info["tuned_tile_width"] == W and info["tuned_chain"] in (sw.CHAIN_TILES, sw.CHAIN_BANDS, sw.CHAIN_RING)
         nsteps = 7 * _sph(wl.EULER, W) + 1
         assert_bits_equal(run_swept(w, np.float64, nsteps, W, (sw.KERNEL_WAVE, info["tuned_chain"])), run_naive(w, np.float64, nsteps), "tuned variant")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# one handle, several streams; grids narrower than the narrowest register tile
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("chain", [sw.CHAIN_RING, sw.CHAIN_BANDS, sw.CHAIN_TILES], ids=["ring", "band", "chain"])
+def test_one_handle_from_two_streams_is_serialised_not_corrupted(chain):
+    """include/swept1d.h: calls on one handle from different streams run one after the other (each call's stream waits for
+    the handle's previous call), so the flags / counters the launch-free kernels share are never re-zeroed under a running
+    kernel.  Two fields advance alternately on two streams through ONE handle; a CUDA graph replay joins in."""
+    import torch
+    w = _noise(wl.HEAT, 1 << 16)
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with solver_for(w, np.float64) as s:
+        s.set_option(sw.OPT_CHAIN, chain)
+        u1, u2 = to_dev(w.initial(np.float64)), to_dev(w.initial(np.float64))
+        torch.cuda.synchronize()
+        for i in range(6):
+            s.set_option(sw.OPT_SWEPT_GRAPH, i % 2)
+            s.swept_run(u1, 700, 256, stream=st1)
+            s.swept_run(u2, 700, 256, stream=st2)
+        s.naive_run(u2, 5, stream=st1)
+        s.naive_run(u1, 5, stream=st2)
+        torch.cuda.synchronize()
+        ref = run_naive(w, np.float64, 6 * 700 + 5)
+        assert_bits_equal(u1.cpu().numpy(), ref, "field 1")
+        assert_bits_equal(u2.cpu().numpy(), ref, "field 2")
+
+
+@pytest.mark.parametrize("problem", PROBLEMS, ids=["heat", "ks", "euler"])
+@pytest.mark.parametrize("nx", [8, 32])
+def test_default_width_on_grids_narrower_than_a_register_tile(problem, nx):
+    """swept_run(tile_width = 0) on a grid too small for the WAVE kernels falls back to the shared-memory kernels."""
+    import torch
+    w = _noise(problem, nx)
+    with solver_for(w, np.float64) as s:
+        u = to_dev(w.initial(np.float64))
+        s.swept_run(u, 23, 0)
+        torch.cuda.synchronize()
+        assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float64, 23), f"default width nx={nx}")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# Euler: the batched reciprocal / square root (stencils.cuh fp<T>::rcp_fast / sqrt_fast) must equal IEEE division and
+# square root for EVERY operand, also those that leave the fast path (subnormal / huge densities, tiny sound speeds)
+# ------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", DTYPES, ids=["f64", "f32"])
+@pytest.mark.parametrize("case", ["tiny-density", "huge-density", "tiny-sound-speed"])
+def test_batched_rcp_sqrt_fallback(case, dtype):
+    nx, nsteps = 2048, 24
+    rng = np.random.default_rng(7)
+    big = 1000 if dtype == np.float64 else 120
+    rho = 1 + 0.3 * rng.uniform(-1, 1, nx)
+    vel = 0.3 * rng.uniform(-1, 1, nx)
+    p = 1 + 0.3 * rng.uniform(-1, 1, nx)
+    if case == "tiny-density":        # rho, m, E all scaled by 2^-big: 1 / rho leaves the fast path's exponent range (f64)
+        scale_rho, scale_p = 2.0 ** -big, 2.0 ** -big
+    elif case == "huge-density":      # 1 / rho is subnormal
+        big = 1022 if dtype == np.float64 else 126
+        scale_rho, scale_p = 2.0 ** big, 2.0 ** big
+        vel, p = 0.01 * vel, 0.01 * p
+    else:                             # c^2 = gamma p / rho below the square root's fast range
+        scale_rho, scale_p = 1.0, 2.0 ** -(big + 10)
+        vel = 0.0 * vel
+    U0 = wl.euler_conserved(rho * scale_rho, vel, p * scale_p).astype(dtype)
+    assert np.all(np.isfinite(U0)) and np.all(U0[0] > 0)
+    w = wl.Workload(wl.EULER, nx, 1.0 / nx, 0.2 / nx, U0.astype(np.float64), name="euler-" + case)
+    ref = run_oracle(w, dtype, nsteps, u0=U0)
+    assert np.all(np.isfinite(ref)) and not np.array_equal(ref, U0)
+    assert_bits_equal(run_naive(w, dtype, nsteps, u0=U0), ref, f"classic vs oracle, {case}")
+    for kernel in (SMEM_V, BAND_V):
+        assert_bits_equal(run_swept(w, dtype, nsteps, 256, kernel, u0=U0), ref, f"swept vs oracle, {case}")
+
+
+# ------------------------------------------------------------------------------------------------------------
+# ring kernel (SWEPT_OPT_CHAIN = 3, the default): communication warp, cp.async-staged exchange, remainder inside the launch
+# ------------------------------------------------------------------------------------------------------------
+RING_CASES = [
+    # problem, dtype, nx, W, q, r                   what it exercises
+    (wl.HEAT, np.float64, 256, 128, 9, 0),          # two bands, each the other's neighbour on both sides; 16-iteration chunks
+    (wl.HEAT, np.float64, 1 << 11, 128, 5, 37),     # odd remainder: truncated closing cycle, final values from two alignments
+    (wl.HEAT, np.float64, 1 << 12, 128, 1, 0),      # q = 1: upright triangle straight into the closing triangle
+    (wl.HEAT, np.float64, 1 << 12, 128, 0, 63),     # q = 0: only the truncated cycle, remainder L - 1
+    (wl.HEAT, np.float64, 1 << 12, 256, 0, 1),
+    (wl.HEAT, np.float64, 1 << 12, 256, 2, 127),
+    (wl.HEAT, np.float32, 1 << 16, 256, 40, 3),     # one band per warp, many phases (SR = 2 iterations)
+    (wl.HEAT, np.float64, 1 << 22, 1024, 5, 336),   # 4096 bands on 148 x 15 warps: 1 or 2 bands per warp, parked columns
+    (wl.HEAT, np.float32, 1 << 22, 256, 5, 100),    # 16384 bands: several bands per warp, rotating parked buffers
+    (wl.HEAT, np.float64, 1 << 21, 128, 6, 11),     # SR = 1 tiles, 16384 bands
+    (wl.HEAT, np.float32, 1 << 22, 512, 5, 255),    # four super-rows per iteration
+    (wl.HEAT, np.float64, 1 << 21, 512, 3, 2),
+    (wl.HEAT, np.float64, 1 << 16, 512, 7, 77),     # roomy build (no more bands than 3 warps per SM)
+    (wl.KS, np.float64, 1 << 14, 256, 11, 5),
+    (wl.KS, np.float32, 1 << 21, 256, 4, 31),       # 8192 bands, several per warp
+    (wl.KS, np.float64, 1 << 20, 1024, 3, 100),
+    (wl.KS, np.float64, 1 << 22, 512, 2, 63),       # the size the band kernel could not hold in shared memory (per-warp packing)
+    (wl.KS, np.float32, 1 << 22, 512, 3, 1),
+    (wl.EULER, np.float64, 1 << 13, 256, 7, 3),
+    (wl.EULER, np.float32, 1 << 20, 256, 3, 17),
+    (wl.EULER, np.float64, 1 << 18, 512, 2, 50),
+    (wl.EULER, np.float64, 1 << 20, 256, 3, 9),     # config 4's largest grid: 4096 bands, parked columns packed per warp
+    (wl.EULER, np.float32, 1 << 21, 512, 2, 0),      # 4096 bands of 3 fields: 3 or 2 bands per warp
+]
+
+
+@pytest.mark.parametrize("problem,dtype,nx,W,q,r", RING_CASES)
+def test_ring_kernel_equals_classic(problem, dtype, nx, W, q, r):
+    import torch
+    w = _noise(problem, nx)
+    assert r < _sph(problem, W)
+    nsteps = q * _sph(problem, W) + r
+    with solver_for(w, dtype) as s:
+        assert s.tile_width_ok(W)
+        u = to_dev(w.initial(dtype))
+        s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        info = s.info()
+        assert info["last_sweep_launch"] == sw.LAUNCH_RING, "this case must run on swept_ring_kernel, not fall back"
+        assert info["launches_last_call"] == 1, "remainder included, a swept_run is one launch"
+        got = u.cpu().numpy()
+    assert_bits_equal(got, run_naive(w, dtype, nsteps), f"ring nx={nx} W={W} q={q} r={r}")
+
+
+def test_ring_repeated_calls_two_handles_two_streams_and_graph_replay():
+    import torch
+    w = _noise(wl.KS, 1 << 18)
+    s1, s2 = solver_for(w, np.float64), solver_for(w, np.float64)
+    s2.set_option(sw.OPT_SWEPT_GRAPH, 1)
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    u1, u2 = to_dev(w.initial(np.float64)), to_dev(w.initial(np.float64))
+    torch.cuda.synchronize()
+    for _ in range(3):
+        s1.swept_run(u1, 333, 256, stream=st1)
+        s2.swept_run(u2, 333, 256, stream=st2)
+    torch.cuda.synchronize()
+    assert s1.info()["last_sweep_launch"] == sw.LAUNCH_RING
+    ref = run_naive(w, np.float64, 999)
+    assert_bits_equal(u1.cpu().numpy(), ref, "stream 1")
+    assert_bits_equal(u2.cpu().numpy(), ref, "stream 2 (graph replay)")
+    s1.close(); s2.close()
