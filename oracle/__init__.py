@@ -29,6 +29,9 @@ def lib() -> ctypes.CDLL:
             f = getattr(L, f"oracle_heat_insulated_{suf}")
             f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double]
             f.restype = ctypes.c_int
+            f = getattr(L, f"oracle_heat2d_{suf}")
+            f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+            f.restype = ctypes.c_int
             f = getattr(L, f"oracle_ks_{suf}")
             f.argtypes = [ptr, ctypes.c_long, ctypes.c_long, ctypes.c_double, ctypes.c_double]
             f.restype = ctypes.c_int
@@ -72,6 +75,19 @@ def heat_insulated(u: np.ndarray, nsteps: int, alpha: float, dx: float, dt: floa
     rc = getattr(lib(), f"oracle_heat_insulated_{suf}")(p, nx, int(nsteps), float(alpha), float(dx), float(dt))
     if rc != 0:
         raise RuntimeError(f"oracle_heat_insulated failed rc={rc}")
+    return a
+
+
+def heat2d(u: np.ndarray, nsteps: int, alpha: float, dx: float, dt: float) -> np.ndarray:
+    """2-D FTCS heat (5-point), periodic in both directions; u has shape [ny, nx] (row-major, x fastest)."""
+    if u.dtype not in (np.float32, np.float64) or u.ndim != 2:
+        raise TypeError("oracle.heat2d takes a 2-D float32 / float64 array [ny, nx]")
+    a = np.array(u, copy=True, order="C")
+    suf = "f64" if a.dtype == np.float64 else "f32"
+    cty = ctypes.c_double if a.dtype == np.float64 else ctypes.c_float
+    rc = getattr(lib(), f"oracle_heat2d_{suf}")(a.ctypes.data_as(ctypes.POINTER(cty)), a.shape[1], a.shape[0], int(nsteps), float(alpha), float(dx), float(dt))
+    if rc != 0:
+        raise RuntimeError(f"oracle_heat2d failed rc={rc}")
     return a
 
 

@@ -7,7 +7,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "swept_oracle.c")]
-DEPS = SRC + [os.path.join(HERE, "schemes.inc")]
+DEPS = SRC + [os.path.join(HERE, "schemes.inc"), os.path.join(HERE, "heat2d.inc")]
 OUT = os.path.join(HERE, "liboracle.so")
 # -ffp-contract=off: no implicit FMA, so the only fused operations are the explicit fma() calls of
 # the canonical order.  No -march flags: the .so is built on one box and run on another.

@@ -23,6 +23,9 @@
  * one-line mutants: zero / maxmod / unlimited slopes, full-step predictor, forward Euler, wrong face
  * sign).  Parity unpinned: none.  (Euler is BASELINE.json config 4's scheme; the paper has none.)
  *
+ * 2-D heat (heat2d.inc) -- separable amplification factor 1-4Fo(sin^2+sin^2), exact lattice-walk delta response
+ * at Fo = 1/4 (binomial closed form), sum conservation, max principle, bitwise transposition symmetry, reduction to the 1-D oracle.
+ *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).  `omp parallel for`
  * over the spatial index is the only parallelism; it does not change any result.
  */
@@ -40,6 +43,7 @@
 #define R_FABS fabs
 #define R_FMAX fmax
 #include "schemes.inc"
+#include "heat2d.inc"
 #undef REAL
 #undef FN
 #undef R_FMA
@@ -54,6 +58,7 @@
 #define R_FABS fabsf
 #define R_FMAX fmaxf
 #include "schemes.inc"
+#include "heat2d.inc"
 #undef REAL
 #undef FN
 #undef R_FMA

@@ -20,7 +20,7 @@ HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", "swept_band.cuh", "sw
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
     "-Xcompiler", "-fPIC,-ffp-contract=off",
-]
+] + os.environ.get("SWEPT_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:
