@@ -31,6 +31,8 @@ SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
     "swept_band_layout", "swept_band_owner", "swept_problem_info",
+    # include/swept2d.h
+    "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_get_info", "swept2d_destroy",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -63,6 +65,15 @@ class _Launch(ctypes.Structure):
 
 class _BandLayout(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int) for n in ("blocks", "warps_per_block", "slots_per_block", "warps_per_slot", "slots", "max_bands_per_warp", "ntiles")]
+
+
+class _Params2D(ctypes.Structure):
+    _fields_ = [("dtype", ctypes.c_int), ("alpha", ctypes.c_double)]
+
+
+class _Info2D(ctypes.Structure):
+    _fields_ = [("dtype", ctypes.c_int), ("nx", ctypes.c_int64), ("ny", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64),
+                ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64)]
 
 
 _lib = None
@@ -99,6 +110,11 @@ def lib() -> ctypes.CDLL:
     L.swept_band_layout.argtypes = [ci, ci, ci, ctypes.POINTER(_BandLayout)]
     L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     L.swept_problem_info.argtypes = [ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
+    L.swept2d_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, ctypes.POINTER(_Params2D)]
+    L.swept2d_run.argtypes = [vp, vp, i64, ci, vp]
+    L.naive2d_run.argtypes = [vp, vp, i64, vp]
+    L.swept2d_get_info.argtypes = [vp, ctypes.POINTER(_Info2D)]
+    L.swept2d_destroy.argtypes = [vp]
     for name in SYMBOLS:
         getattr(L, name).restype = ci
     L.swept_plan.restype = i64
@@ -206,6 +222,56 @@ class Solver:
     def close(self) -> None:
         if getattr(self, "_h", None) is not None and self._h.value:
             lib().swept_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Solver2D:
+    """One `swept2d_create` handle (include/swept2d.h): the 2-D heat equation on a periodic nx x ny grid.  `u` arguments are
+    contiguous CUDA tensors of shape [ny, nx] of the handle's dtype, advanced IN PLACE and asynchronously on `stream`."""
+
+    def __init__(self, nx: int, ny: int, dx: float, dt: float, *, dtype=F64, alpha: float = 1.0):
+        self._h = ctypes.c_void_p()
+        self.nx, self.ny, self.dtype = int(nx), int(ny), _dtype_id(dtype)
+        p = _Params2D(self.dtype, float(alpha))
+        _check(lib().swept2d_create(ctypes.byref(self._h), self.nx, self.ny, float(dx), float(dt), ctypes.byref(p)))
+        import torch
+        self.device = torch.cuda.current_device()
+
+    def _ptr(self, u) -> int:
+        import torch
+        want = torch.float64 if self.dtype == F64 else torch.float32
+        if not (isinstance(u, torch.Tensor) and u.is_cuda and u.is_contiguous() and u.dtype == want):
+            raise SweptError(EINVAL, "u must be a contiguous CUDA tensor of the handle's dtype")
+        if u.device.index != self.device or u.numel() != self.nx * self.ny:
+            raise SweptError(EINVAL, f"u must hold ny*nx = {self.nx * self.ny} elements on cuda:{self.device}")
+        return u.data_ptr()
+
+    def swept_run(self, u, nsteps: int, tile_width: int = 0, stream=None) -> None:
+        _check(lib().swept2d_run(self._h, self._ptr(u), int(nsteps), int(tile_width), _stream_ptr(stream)))
+
+    def naive_run(self, u, nsteps: int, stream=None) -> None:
+        _check(lib().naive2d_run(self._h, self._ptr(u), int(nsteps), _stream_ptr(stream)))
+
+    def info(self) -> dict:
+        i = _Info2D()
+        _check(lib().swept2d_get_info(self._h, ctypes.byref(i)))
+        return {name: getattr(i, name) for name, _ in _Info2D._fields_}
+
+    def close(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().swept2d_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __enter__(self):

@@ -12,8 +12,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libswept1d.so")
 SOURCES = ["api.cu", "naive.cu", "swept_smem.cu", "swept_wave.cu", "swept_wave_heat.cu", "swept_wave_ks.cu", "swept_wave_euler.cu",
-           "swept_band_heat.cu", "swept_band_ks.cu", "swept_band_euler.cu", "swept_ring_heat.cu", "swept_ring_ks.cu", "swept_ring_euler.cu", "alu_peak.cu"]
-HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", "swept_band.cuh", "swept_ring.cuh", os.path.join("..", "..", "include", "swept1d.h")]
+           "swept_band_heat.cu", "swept_band_ks.cu", "swept_band_euler.cu", "swept_ring_heat.cu", "swept_ring_ks.cu", "swept_ring_euler.cu", "heat2d.cu", "alu_peak.cu"]
+HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", "swept_band.cuh", "swept_ring.cuh", os.path.join("..", "..", "include", "swept1d.h"), os.path.join("..", "..", "include", "swept2d.h")]
 # -fmad=false: no implicit FMA contraction -- the only fused operations are the explicit fma() calls of the
 # canonical evaluation order, so classic, swept and the CPU oracle round identically.
 # Default -prec-div=true -prec-sqrt=true -ftz=false are kept (IEEE division and square root, denormals).

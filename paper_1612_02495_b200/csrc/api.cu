@@ -51,6 +51,14 @@ static int fail_cuda(cudaError_t e, const char *what) {
     return fail(SWEPT_ECUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+int swept::swept_fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
 extern "C" const char *swept_last_error(void) { return g_err; }
 extern "C" const char *swept_version(void) { return "swept1d-b200 0.1 (sm_100a)"; }
 

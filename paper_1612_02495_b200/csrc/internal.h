@@ -89,6 +89,9 @@ __host__ __device__ inline void band_owner(const BandGrid &g, int band, int *blo
     *index = round / g.wps;
 }
 
+// Record an error message for swept_last_error() (thread-local, api.cu) and return `code`.
+int swept_fail(int code, const char *fmt, ...) __attribute__((format(printf, 2, 3)));
+
 // FMA-chain microbenchmark (alu_peak.cu)
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st);
 

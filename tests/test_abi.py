@@ -1,4 +1,4 @@
-"""The C-ABI library builds, loads and exports every symbol include/swept1d.h declares; no compute calls (no GPU)."""
+"""The C-ABI library builds, loads and exports every symbol include/*.h declares; no compute calls (no GPU)."""
 import ctypes
 import os
 import re
@@ -8,11 +8,11 @@ import pytest
 import paper_1612_02495_b200 as sw
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-HEADER = os.path.join(ROOT, "include", "swept1d.h")
+HEADERS = [os.path.join(ROOT, "include", "swept1d.h"), os.path.join(ROOT, "include", "swept2d.h")]
 
 
 def _declared_functions():
-    src = open(HEADER).read()
+    src = "\n".join(open(h).read() for h in HEADERS)
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     names = re.findall(r"^\s*(?:const\s+char\s*\*|int64_t|int)\s*\**\s*(\w+)\s*\(", src, flags=re.M)
     return sorted(set(names))

@@ -1,0 +1,96 @@
+"""Host logic of the 2-D swept rule, checked on a plain-Python integer model before any kernel.
+
+Decomposition: in each direction the 1-D swept rule partitions the axis, at local tier s = 1..L of a
+half-cycle (L = W/2), into the shrinking intervals U(s) = [s, W - s) of the tiles of one alignment and the expanding intervals
+D(s) = [c - s, c + s), c = W/2, of the tiles shifted by W/2 (Fig. 1).  The 2-D rule is the product: every point is,
+at tier s, in exactly one of U x U (pyramid), D x U / U x D (the two bridges), D x D (inverted pyramid), and the 5-point stencil makes
+U x U self-contained, the bridges depend on U x U, and D x D on all three.  D x D of one half-cycle and U x U of the next sit on the
+same (shifted) tiles and fuse into an octahedron, so a half-cycle is TWO launches: bridges, octahedra.  Values live in two
+arrays, P0 (newest even tier at every point) and P1 (newest odd tier) -- the 2-D form of the in-place staircase rows R0 / R1.
+"""
+import numpy as np
+import pytest
+
+
+class Model2D:
+    """Integer 5-point stencil new = c0 u + (E + W + N + S) on a periodic [ny][nx] grid; P[0] / P[1] hold even / odd tiers."""
+
+    def __init__(self, nx, ny, u0):
+        self.nx, self.ny = nx, ny
+        self.P = [np.array(u0, dtype=object).reshape(ny, nx), np.zeros((ny, nx), dtype=object)]
+        self.updates = 0
+
+    @staticmethod
+    def point(u, e, w, n, s):
+        return 3 * u + ((e + w) + (n + s))
+
+    def naive(self, nsteps):
+        a = self.P[0].copy()
+        for _ in range(nsteps):
+            a = 3 * a + ((np.roll(a, -1, 1) + np.roll(a, 1, 1)) + (np.roll(a, -1, 0) + np.roll(a, 1, 0)))
+        return a
+
+    def region(self, W, ox, oy, mx, my, tiers):
+        """One launch: every tile of the grid shifted by (ox, oy) runs the local tiers `tiers` (1..2L-1; s > L continues as the
+        next half-cycle's U x U) on the rectangle rect_x(s) x rect_y(s), mx / my in 'U', 'D'.  Snapshot semantics: all tiles load
+        before any stores; a tile stores only the points it updated (both planes where it wrote both)."""
+        nx, ny, L, c = self.nx, self.ny, W // 2, W // 2
+
+        def rect(mode, s):
+            if s > L:                       # the shrinking half of an octahedron: local tier s - L of U
+                return (s - L, W - (s - L))
+            return (s, W - s) if mode == "U" else (c - s, c + s)
+
+        stores = []
+        for ty in range(ny // W):
+            for tx in range(nx // W):
+                gx0, gy0 = tx * W + ox, ty * W + oy
+                pl = [{(x, y): self.P[p][(gy0 + y) % ny, (gx0 + x) % nx] for x in range(-1, W + 1) for y in range(-1, W + 1)} for p in (0, 1)]
+                wrote = {}
+                for s in tiers:
+                    (xa, xb), (ya, yb) = rect(mx, s), rect(my, s)
+                    src, dst = pl[(s - 1) & 1], pl[s & 1]
+                    new = {(x, y): self.point(src[x, y], src[x + 1, y], src[x - 1, y], src[x, y + 1], src[x, y - 1])
+                           for x in range(xa, xb) for y in range(ya, yb)}
+                    dst.update(new)
+                    self.updates += len(new)
+                    for k in new:
+                        wrote.setdefault(k, set()).add(s & 1)
+                stores.append((gx0, gy0, pl, wrote))
+        for gx0, gy0, pl, wrote in stores:
+            for (x, y), planes in wrote.items():
+                for p in planes:
+                    self.P[p][(gy0 + y) % ny, (gx0 + x) % nx] = pl[p][x, y]
+
+    def swept(self, W, K):
+        """K half-cycles of L = W/2 timesteps: pyramids, then per half-cycle bridges + octahedra (the last one only its lower half)."""
+        L, h = W // 2, W // 2
+        self.region(W, 0, 0, "U", "U", range(1, L))                                  # upright pyramids from the flat field
+        for k in range(K):
+            a = (k % 2) * h                                                          # alignment that shrinks in this half-cycle
+            b = h - a
+            self.region(W, b, a, "D", "U", range(1, L + 1))                          # bridges: expanding in x, shrinking in y
+            self.region(W, a, b, "U", "D", range(1, L + 1))                          # ... and the other way round (same launch)
+            self.region(W, b, b, "D", "D", range(1, L + 1) if k == K - 1 else range(1, 2 * L))   # inverted pyramids / octahedra
+
+
+@pytest.mark.parametrize("nx,ny,W,K", [(16, 16, 8, 1), (16, 16, 8, 2), (16, 8, 8, 3), (8, 8, 8, 2), (24, 16, 8, 4), (16, 16, 16, 2), (32, 16, 16, 3)])
+def test_2d_swept_plan_on_the_model_equals_naive_stepping(nx, ny, W, K):
+    rng = np.random.default_rng(1612)
+    u0 = [int(v) for v in rng.integers(-5, 6, nx * ny)]
+    m = Model2D(nx, ny, u0)
+    m.swept(W, K)
+    ref = Model2D(nx, ny, u0).naive(K * (W // 2))
+    assert np.array_equal(m.P[0], ref)
+    assert m.updates == nx * ny * K * (W // 2)          # every (point, tier) exactly once
+
+
+def test_region_volumes():
+    """Per tile and half-cycle: pyramid + two bridges + inverted pyramid = L W^2 point updates (the four products of the 1-D
+    triangles' row lengths sum to W x W at every tier)."""
+    for W in (8, 16, 32, 64):
+        L, c = W // 2, W // 2
+        uu = sum((W - 2 * s) ** 2 for s in range(1, L + 1))
+        du = sum(2 * s * (W - 2 * s) for s in range(1, L + 1))
+        dd = sum((2 * s) ** 2 for s in range(1, L + 1))
+        assert uu + 2 * du + dd == L * W * W

@@ -1,0 +1,86 @@
+"""-m gpu parity of the 2-D swept rule (include/swept2d.h): classic 2-D kernel == CPU oracle and swept == classic, bit for bit."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1612_02495_b200 as sw
+import workloads as wl
+from gpu_util import TOL, assert_bits_equal, rel_max, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def _run(nx, ny, dtype, nsteps, W=None, fo=0.2, u0=None):
+    import torch
+    dx, dt = wl.heat2d_grid(max(nx, ny), fo)
+    u0 = wl.heat2d_field(nx, ny).astype(dtype) if u0 is None else u0
+    with sw.Solver2D(nx, ny, dx, dt, dtype=sw.F64 if dtype == np.float64 else sw.F32) as s:
+        u = to_dev(u0)
+        if W is None:
+            s.naive_run(u, nsteps)
+        else:
+            s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        return u.cpu().numpy(), s.info()
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("nx,ny,nsteps", [(8, 8, 3), (64, 32, 37), (256, 512, 20)])
+def test_classic_2d_matches_oracle(nx, ny, nsteps, dtype):
+    got, _ = _run(nx, ny, dtype, nsteps)
+    dx, dt = wl.heat2d_grid(max(nx, ny), 0.2)
+    ref = oracle.heat2d(wl.heat2d_field(nx, ny).astype(dtype), nsteps, 1.0, dx, dt)
+    assert rel_max(got[None], ref[None]) <= TOL[dtype]
+    assert_bits_equal(got, ref, f"classic 2-D vs oracle {nx}x{ny}")
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32], ids=["f64", "f32"])
+@pytest.mark.parametrize("nx,ny,W,nsteps", [
+    (8, 8, 8, 4),            # one tile wrapping onto itself in both directions, one half-cycle
+    (16, 8, 8, 4 * 3 + 1),   # three half-cycles (closes on the shifted alignment) + a remainder step
+    (64, 128, 16, 8 * 4),    # even half-cycle count
+    (128, 64, 32, 16 * 2 + 7),
+    (512, 512, 32, 16 * 5 + 3),
+    (256, 1024, 16, 8 * 7),
+])
+def test_swept_2d_equals_classic_and_oracle(nx, ny, W, nsteps, dtype):
+    got, info = _run(nx, ny, dtype, nsteps, W=W)
+    ref, _ = _run(nx, ny, dtype, nsteps)
+    L = W // 2
+    assert info["launches_last_call"] == nsteps % L + 1 + 2 * (nsteps // L)       # remainder + pyramids + (bridges, octahedra) per half-cycle
+    assert_bits_equal(got, ref, f"swept 2-D vs classic {nx}x{ny} W={W}")
+    dx, dt = wl.heat2d_grid(max(nx, ny), 0.2)
+    orc = oracle.heat2d(wl.heat2d_field(nx, ny).astype(dtype), nsteps, 1.0, dx, dt)
+    assert rel_max(got[None], orc[None]) <= TOL[dtype]
+    assert_bits_equal(got, orc, "swept 2-D vs oracle")
+
+
+def test_swept_2d_full_size_sampled_against_the_oracle():
+    """nx = ny = 4096 (128 MiB of fp64: HBM-resident), 400 timesteps: whole field == classic; the oracle on a periodic window whose
+    centre block lies outside the reach of the window's seam."""
+    n, nsteps, M = 4096, 400, 1024
+    rng = np.random.default_rng(3)
+    u0 = rng.uniform(-1, 1, (n, n))
+    got, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0)
+    ref, _ = _run(n, n, np.float64, nsteps, u0=u0)
+    assert_bits_equal(got, ref, "swept 2-D vs classic at 4096^2")
+    dx, dt = wl.heat2d_grid(n, 0.2)
+    for cy, cx in ((0, 0), (n // 2 + 16, n // 2 + 16)):
+        iy, ix = (cy - M // 2 + np.arange(M)) % n, (cx - M // 2 + np.arange(M)) % n
+        win = oracle.heat2d(np.ascontiguousarray(u0[np.ix_(iy, ix)]), nsteps, 1.0, dx, dt)
+        V = M // 2 - nsteps - 8
+        keep = np.arange(M // 2 - V, M // 2 + V)
+        assert_bits_equal(got[np.ix_(iy[keep], ix[keep])], win[np.ix_(keep, keep)], f"oracle window at ({cy}, {cx})")
+
+
+def test_illegal_arguments_2d():
+    with pytest.raises(sw.SweptError):
+        sw.Solver2D(100, 64, 0.01, 1e-5)
+    dx, dt = wl.heat2d_grid(64)
+    with sw.Solver2D(64, 64, dx, dt) as s:
+        u = to_dev(wl.heat2d_field(64, 64))
+        for bad in (4, 12, 64, -8):
+            with pytest.raises(sw.SweptError):
+                s.swept_run(u, 10, bad)
+        with pytest.raises(sw.SweptError):
+            s.naive_run(u.float(), 1)

@@ -210,3 +210,20 @@ def make(problem, nx: int, kind: str = "config") -> Workload:
 def steps_per_half_cycle(problem: int, tile_width: int) -> int:
     """L/S: full timesteps one swept half-cycle advances (SURVEY §8 notation)."""
     return tile_width // (2 * RADIUS[problem] * STAGES[problem])
+
+
+# ----------------------------------------------------------------------------------------------
+# 2-D heat (SURVEY.md section 8(f) NEXT-4): inputs only -- a seeded smooth field plus grid-scale noise on [0,1)^2
+# ----------------------------------------------------------------------------------------------
+def heat2d_grid(n: int, fo: float = 0.25):
+    """dx = dy = 1/n, alpha = 1, dt = fo dx^2 (fo = 1/4 is the stability limit of the 5-point FTCS scheme)."""
+    dx = 1.0 / n
+    return dx, fo * dx * dx
+
+
+def heat2d_field(nx: int, ny: int, seed: int = SEED_NOISE, noise: float = 1.0) -> np.ndarray:
+    """sin(2 pi x) cos(4 pi y) + noise * U[-1,1] grid-scale noise, float64 [ny, nx]."""
+    x = (np.arange(nx) + 0.5) / nx
+    y = (np.arange(ny) + 0.5) / ny
+    smooth = np.sin(2 * np.pi * x)[None, :] * np.cos(4 * np.pi * y)[:, None]
+    return np.ascontiguousarray(smooth + noise * np.random.default_rng(seed).uniform(-1.0, 1.0, (ny, nx)))
