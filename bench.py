@@ -92,9 +92,12 @@ def parse():
                     help="launch-free sweep: 3 = ring kernel (default: bands + communication warp, remainder inside the launch), 2 = streaming bands, "
                          "1 = tile flags, 0 = one launch per half-cycle (PAPER.md:98)")
     ap.add_argument("--no-chain", action="store_true", help="same as --chain 0")
+    ap.add_argument("--pack", type=int, default=0, choices=[0, 1, 2], help="SWEPT_OPT_PACK (heat fp32, band kernel): 0 auto / tuned, 1 off, 2 packed pairs of bands")
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="SWEPT_OPT_BLOCKS_PER_SM for the per-tile kernels (0 = none / tuned)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
+    ap.add_argument("--heat2d", action="store_true", help="secondary measurement (SURVEY.md section 8(f) NEXT-4): the 2-D swept rule against the classic "
+                    "2-D kernel on an nx x nx periodic grid (--nx, default 8192; --nsteps, default 800), one JSON line")
     return ap.parse_args()
 
 
@@ -408,8 +411,61 @@ def run_stress(args):
               f"{bk('ring')} | {bk('band')} | {bk('chain')} | {bk('smem')} |")
 
 
+def run_heat2d(args):
+    """2-D heat, fp64 / fp32, nx x nx (HBM-resident at the default 8192^2 = 512 MiB): swept (W = 32, 16) vs classic, CUDA-event timed."""
+    import torch
+
+    import paper_1612_02495_b200 as sw
+
+    torch.cuda.set_device(0)
+    n = args.nx if args.nx != (1 << 22) else 8192
+    nsteps = args.nsteps or 800
+    np_dtype = np.float64 if args.dtype == "f64" else np.float32
+    dx, dt = wl.heat2d_grid(n, 0.2)
+    u0 = torch.from_numpy(wl.heat2d_field(n, n).astype(np_dtype)).cuda()
+    u = u0.clone()
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        fn()
+        ts = []
+        for _ in range(max(args.steps, 3)):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream); e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        return statistics.median(ts)
+
+    res = {}
+    with sw.Solver2D(n, n, dx, dt, dtype=sw.F64 if args.dtype == "f64" else sw.F32) as s:
+        t = timed(lambda: s.naive_run(u, nsteps))
+        res["classic"] = n * n * nsteps / t / 1e9
+        for W in (32, 16, 8):
+            u.copy_(u0)
+            t = timed(lambda: s.swept_run(u, nsteps, W))
+            res[f"swept W={W}"] = n * n * nsteps / t / 1e9
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_peak = 6650.0
+    es = u.element_size()
+    best = max((k for k in res if k.startswith("swept")), key=res.get)
+    print(json.dumps({
+        "metric": "grid-point updates/sec (2-D heat, secondary)", "unit": "GPts*steps/s", "value": res[best], "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": f"2-D heat FTCS 5-point, periodic {n} x {n}, Fo = 0.2, {nsteps} timesteps; field {n * n * es >> 20} MiB (larger than L2)", "best": best},
+        "results": res, "speedup_swept_over_classic": res[best] / res["classic"],
+        "classic_roofline": {"bound": "hbm", "algorithmic_bytes_per_update": 2 * es, "achieved_GBps": res["classic"] * 2 * es, "peak_GBps": hbm_peak,
+                             "frac": res["classic"] * 2 * es / hbm_peak},
+        # swept: per half-cycle of L = W/2 timesteps the two launches (bridges, octahedra) each read both arrays over every tile
+        # box and write what they updated: about 4 reads + 3 writes per point = 7 values per L timesteps
+        "swept_hbm_algorithmic_bytes_per_update": {f"W={W}": 7 * es / (W // 2) for W in (32, 16, 8)},
+    }))
+
+
 def main():
     args = parse()
+    if args.heat2d:
+        run_heat2d(args)
+        return
     if args.impl == "reference":
         run_reference(args)
         return
@@ -445,6 +501,8 @@ def main():
     s.set_option(sw.OPT_CHAIN, chain_opt)
     if args.blocks_per_sm:
         s.set_option(sw.OPT_BLOCKS_PER_SM, args.blocks_per_sm)
+    if args.pack:
+        s.set_option(sw.OPT_PACK, args.pack)
     if not any(s.tile_width_ok(W) for W in (32, 64, 128, 256, 512, 1024)):
         kernel = sw.KERNEL_SMEM
         s.set_option(sw.OPT_KERNEL, kernel)
@@ -571,6 +629,17 @@ def main():
         # upper-right edge (2 W values: lane 31's row outputs out, lane 0's row feed in)
         "hbm_algorithmic_bytes_per_launch": int((2 if band else 4) * w.nx * pinfo["ncomp"] * u.element_size() * hc),
     }
+    # shared-memory roofline (north_star: "shared-memory throughput for the swept path ... against the chip's peak"): it bounds the
+    # paper-style kernels, which move (2h + 1) loads + 1 store of shared memory per point update; the register kernels touch
+    # shared memory only for the edge rings (2 s / PW bytes per update and less)
+    smem_peak = sw.measure_smem_peak()["bytes_per_s"]
+    roofline["smem_peak_measured_GBps"] = smem_peak / 1e9
+    roofline["smem_peak_nominal_GBps"] = 148 * 128 * 1.965
+    if kernel == sw.KERNEL_SMEM:
+        smem_bytes = (2 * H + 2) * pinfo["ncomp"] * u.element_size() * stage_updates
+        roofline["smem_achieved_GBps"] = smem_bytes / t_launch / 1e9
+        roofline["smem_frac"] = smem_bytes / t_launch / smem_peak
+        roofline["bound"] = "smem"
 
     # ---- classic path on the same workload (context: swept / classic speedup) ------------------------------
     classic = None
@@ -612,7 +681,7 @@ def main():
             "nx": w.nx, "nsteps_per_step": w.nsteps, "boundary": args.boundary, "tile_width": W,
             "kernel": (lname if chain else "wave") if kernel == sw.KERNEL_WAVE else "smem",
             "tile_width_source": "--tile-width" if args.tile_width else "swept_tune, before the timed region",
-            "tune_ms": tune_ms, "tune_launches": int(tune_launches),
+            "tune_ms": tune_ms, "tune_launches": int(tune_launches), "tuned_pack": s.info()["tuned_pack"],
             "parallelism": "replicas only" if world > 1 else "1 GPU",
             "l2": "L2 flushed (256 MB write) between timed steps; the 32 MiB field is L2-resident within a step by the config's size",
         },

@@ -75,6 +75,11 @@ enum {
                                      block per SM, caps its warps at 4 x this), 0 = none / the tuner's choice        */
     SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
     SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
+    SWEPT_OPT_PACK = 6,           /* heat fp32 on the streaming band kernel: 2 = every warp slot advances TWO bands (half a domain
+                                     apart) in lock step on packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: half the FP
+                                     instructions, per-component IEEE rounding, so the result is bit-identical); 1 = one band
+                                     per slot; 0 (default) = swept_tune's measurement for the tuned width, else on when every
+                                     SM gets at least sixteen bands                                                   */
     SWEPT_OPT_CHAIN = 5           /* WAVE kernels, launch-free sweep (beyond the paper; removes PAPER.md:232's launch / wave
                                      costs): ONE persistent launch runs all half-cycles of a swept_run.
                                      3 (default) = streaming bands with a communication warp per block: as 2, but the edge
@@ -139,6 +144,8 @@ typedef struct {
                                     under the default option 3; 0 = not tuned                                        */
     int tuned_blocks_per_sm;     /* resident-blocks cap swept_tune measured as fastest for tuned_tile_width when called with
                                     blocks_per_sm_cap = 0 (0 = none); used while SWEPT_OPT_BLOCKS_PER_SM is 0          */
+    int tuned_pack;              /* SWEPT_OPT_PACK value (1 | 2) swept_tune measured as faster for the tuned width and kernel;
+                                    0 = not measured (not heat fp32 on the band kernel)                              */
 } swept_info_t;
 
 /* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's
@@ -224,6 +231,11 @@ int swept_tile_width_ok(swept_handle_t h, int tile_width);
  * FP instr/s) in *instr_per_s and the elapsed milliseconds of the timed launch in *ms (may be
  * NULL).  SYNCHRONISES.  Used by bench.py for the "alu" roofline denominator. */
 int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms, void *cuda_stream);
+
+/* Measure the shared-memory read peak the paper-style kernels are bound by: conflict-free 16-byte loads by every thread of
+ * every SM; returns bytes per second in *bytes_per_s (nominal: 128 B per clock per SM) and the milliseconds of the timed launch
+ * in *ms (may be NULL).  SYNCHRONISES. */
+int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cuda_stream);
 
 /* Free the workspace and the handle.  The caller must have synchronised every stream it used. */
 int swept_destroy(swept_handle_t h);

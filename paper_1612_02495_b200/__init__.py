@@ -18,7 +18,8 @@ from typing import Optional
 HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
-OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN = 0, 1, 2, 3, 4, 5
+OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN, OPT_PACK = 0, 1, 2, 3, 4, 5, 6
+PACK_AUTO, PACK_OFF, PACK_ON = 0, 1, 2
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}
 BC_PERIODIC, BC_INSULATED = 0, 1
@@ -30,7 +31,7 @@ PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
 SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
-    "swept_band_layout", "swept_band_owner", "swept_problem_info",
+    "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak",
     # include/swept2d.h
     "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_get_info", "swept2d_destroy",
 )
@@ -56,6 +57,7 @@ class _Info(ctypes.Structure):
         ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
         ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int), ("boundary", ctypes.c_int), ("tuned_chain", ctypes.c_int), ("tuned_blocks_per_sm", ctypes.c_int),
+        ("tuned_pack", ctypes.c_int),
     ]
 
 
@@ -110,6 +112,7 @@ def lib() -> ctypes.CDLL:
     L.swept_band_layout.argtypes = [ci, ci, ci, ctypes.POINTER(_BandLayout)]
     L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     L.swept_problem_info.argtypes = [ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
+    L.swept_measure_smem_peak.argtypes = [ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     L.swept2d_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, ctypes.POINTER(_Params2D)]
     L.swept2d_run.argtypes = [vp, vp, i64, ci, vp]
     L.naive2d_run.argtypes = [vp, vp, i64, vp]
@@ -292,6 +295,13 @@ def measure_alu_peak(dtype=F64, stream=None) -> dict:
     ips, ms = ctypes.c_double(0), ctypes.c_double(0)
     _check(lib().swept_measure_alu_peak(_dtype_id(dtype), ctypes.byref(ips), ctypes.byref(ms), _stream_ptr(stream)))
     return {"instr_per_s": ips.value, "ms": ms.value}
+
+
+def measure_smem_peak(stream=None) -> dict:
+    """Shared-memory read microbenchmark: bytes per second of conflict-free 16-byte loads on every SM."""
+    bps, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().swept_measure_smem_peak(ctypes.byref(bps), ctypes.byref(ms), _stream_ptr(stream)))
+    return {"bytes_per_s": bps.value, "ms": ms.value}
 
 
 def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: int = CHAIN_RING) -> list:

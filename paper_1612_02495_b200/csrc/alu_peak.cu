@@ -53,6 +53,55 @@ template <class T> static cudaError_t run_peak(int sm_count, double *instr_per_s
     return cudaSuccess;
 }
 
+// Shared-memory read peak: every thread reads 16 bytes per instruction (LDS.128, consecutive threads consecutive addresses:
+// conflict-free), 8 independent loads in flight; nominal 128 B per clock per SM (B300_MICROARCH guide: smem crossbar).
+__global__ void __launch_bounds__(1024) smem_peak_kernel(float *out, int iters) {
+    __shared__ float4 buf[2048];                                      // 32 KB
+    for (int i = threadIdx.x; i < 2048; i += blockDim.x) buf[i] = make_float4((float)i, 1.f, 2.f, 3.f);
+    __syncthreads();
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    int idx = threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const float4 v = buf[(idx + 256 * k) & 2047];
+            acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
+        }
+        idx = (idx + 32) & 2047;
+    }
+    if (acc.x + acc.y + acc.z + acc.w == 123456789.f) out[0] = acc.x;   // keeps the loads alive
+}
+
+cudaError_t run_smem_peak(int sm_count, double *bytes_per_s, double *ms_out, cudaStream_t st) {
+    float *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, sizeof(float));
+    if (e != cudaSuccess) return e;
+    const int blocks = sm_count * 2, threads = 1024, iters = 4096;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, st);
+        smem_peak_kernel<<<blocks, threads, 0, st>>>(d, iters);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    if (e != cudaSuccess) return e;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (bytes_per_s) *bytes_per_s = (double)blocks * threads * (double)iters * 8 * 16 / (best * 1e-3);
+    if (ms_out) *ms_out = best;
+    return cudaSuccess;
+}
+
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st) {
     return dtype == SWEPT_F64 ? run_peak<double>(sm_count, instr_per_s, ms, st) : run_peak<float>(sm_count, instr_per_s, ms, st);
 }

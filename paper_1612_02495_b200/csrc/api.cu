@@ -22,7 +22,7 @@ struct swept_ctx {
     size_t field_bytes;    // NC*nx*sizeof(T)
     void *host_stage;      // device buffer for swept_run_host (allocated on first use)
     int device, sm_count, max_smem;
-    int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block;
+    int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block, pack, tuned_pack;
     void *sync_base;       // SYNC_HEADER bytes (word 0: the abort word of the bounded waits, swept_wave.cuh) + the sync area
     void *sync;            // sync area = sync_base + SYNC_HEADER; chain kernel: work counter (8 bytes) + done[] flags; band kernel: prog[]
     unsigned *abort_seen;  // pinned host copy of the abort word, refreshed by an async copy behind every launch-free launch
@@ -416,6 +416,7 @@ extern "C" int64_t swept_plan(int problem, int dtype, int64_t nx, int64_t nsteps
 }
 
 static int effective_cap(const swept_ctx *h, int W);
+static int effective_pack(const swept_ctx *h, int W);
 
 static cudaError_t launch_phase(swept_ctx *h, int kernel, int mode, void *d_u, int W, int64_t offset, cudaStream_t st) {
     if (kernel == SWEPT_KERNEL_SMEM) return launch_swept_smem(h->problem, h->dtype, mode, d_u, h->work, h->nx, W, offset, h->cb, st);
@@ -430,6 +431,15 @@ static int effective_chain(const swept_ctx *h, int W) {
 }
 
 // Resident-blocks cap for width W: the option if set, else the cap the tuner measured as fastest for the tuned width.
+// Packed pairs of bands (heat fp32, band kernel): the option if set (1 = off, 2 = on); with 0 (auto) the tuner's measurement for the
+// tuned width, else on where every SM gets at least sixteen bands (enough pairs to fill its warps).
+static int effective_pack(const swept_ctx *h, int W) {
+    if (h->problem != SWEPT_HEAT || h->dtype != SWEPT_F32) return 0;
+    if (h->pack) return h->pack == 2;
+    if (h->tuned_pack && W == h->tuned_tile_width) return h->tuned_pack == 2;
+    return h->nx / W >= (int64_t)16 * h->sm_count;
+}
+
 static int effective_cap(const swept_ctx *h, int W) {
     if (h->blocks_per_sm == 0 && h->tuned_cap && W == h->tuned_tile_width) return h->tuned_cap;
     return h->blocks_per_sm;
@@ -465,7 +475,7 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
             case SWEPT_LAUNCH_BAND:
                 // bands wrap around the periodic domain; a rod with insulated ends runs on the tile-flag kernel
                 e = h->bc ? cudaErrorNotSupported
-                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, 4 * effective_cap(h, L.tile_width), st);
+                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, 4 * effective_cap(h, L.tile_width), effective_pack(h, L.tile_width), st);
                 if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
                 cudaGetLastError();
                 /* the band schedule does not fit this device / size: same half-cycles through the tile-flag kernel */
@@ -527,13 +537,16 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     int wtop = 0;
     for (int W = 4 * h->H; W <= wmax; W <<= 1) if (check_width(h, W, h->kernel, false)) wtop = W;
     if (!wtop) { h->blocks_per_sm = saved_cap; h->swept_graph = saved_graph; return fail(SWEPT_EINVAL, "swept_tune: no legal tile width"); }
-    // every candidate advances the same number of timesteps: twelve half-cycles of the widest tile (long enough that the
-    // first and last phase and the one-off wavefront fill of the launch-free kernels do not decide the ranking)
-    const int64_t nsteps = 12 * (int64_t)(wtop / (2 * h->H * h->S));
+    // every candidate advances the same number of timesteps: 24 half-cycles of the widest tile (long enough that the first and last
+    // phase -- half a phase of work each -- and the one-off wavefront fill of the launch-free kernels do not decide the ranking:
+    // with twelve, heat fp32 at nx = 2^22 was tuned to W = 512 although W = 1024 is 6 % faster over a 50 000-step run)
+    const int64_t nsteps = 24 * (int64_t)(wtop / (2 * h->H * h->S));
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    int best = 0, best_chain = 0, best_cap = 0;
+    int best = 0, best_chain = 0, best_cap = 0, best_pack = 0;
+    const int saved_pack = h->pack;
+    h->tuned_pack = 0;
     float best_ms = 1e30f;
     cudaError_t e = cudaSuccess;
     const int saved_chain = h->chain;
@@ -553,19 +566,25 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
             for (int ci = 0; ci < ncaps && e == cudaSuccess; ++ci) {
                 const int cap = ncaps == 1 ? blocks_per_sm_cap : caps_auto[ci];
                 h->blocks_per_sm = cap;
-                float ms_min = 1e30f;
-                for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
-                    int64_t l = 0;
-                    cudaEventRecord(e0, st);
-                    e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
-                    cudaEventRecord(e1, st);
-                    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
-                    float ms = 0;
-                    if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
-                    if (rep > 0 && ms < ms_min) ms_min = ms;
-                    h->launches_total += l;
+                // heat fp32 on the band kernel: one band per warp slot, and packed pairs
+                const int npack = (saved_pack == 0 && mode == 2 && wave && h->problem == SWEPT_HEAT && h->dtype == SWEPT_F32) ? 2 : 1;
+                for (int pi = 0; pi < npack && e == cudaSuccess; ++pi) {
+                    if (npack == 2) h->pack = 1 + pi;
+                    float ms_min = 1e30f;
+                    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // rep 0 warms up
+                        int64_t l = 0;
+                        cudaEventRecord(e0, st);
+                        e = enqueue_swept(h, h->kernel, d_u_scratch, nsteps, W, st, &l);
+                        cudaEventRecord(e1, st);
+                        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+                        float ms = 0;
+                        if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+                        if (rep > 0 && ms < ms_min) ms_min = ms;
+                        h->launches_total += l;
+                    }
+                    if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = mode; best_cap = cap; best_pack = npack == 2 ? h->pack : 0; }
                 }
-                if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = mode; best_cap = cap; }
+                h->pack = saved_pack;
             }
         }
     }
@@ -580,6 +599,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     h->tuned_tile_width = best;
     h->tuned_chain = (saved_chain == 3 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
     h->tuned_cap = blocks_per_sm_cap == 0 ? best_cap : 0;
+    h->tuned_pack = best_pack;
     if (best_tile_width) *best_tile_width = best;
     return SWEPT_OK;
 }
@@ -628,6 +648,11 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
             if (value < 0 || value > 3) return fail(SWEPT_EINVAL, "swept_set_option: CHAIN takes 0, 1, 2 or 3");
             h->chain = value;
             return SWEPT_OK;
+        case SWEPT_OPT_PACK:
+            if (value < 0 || value > 2) return fail(SWEPT_EINVAL, "swept_set_option: PACK takes 0 (auto), 1 (off) or 2 (on)");
+            h->pack = value;
+            drop_graphs(h);
+            return SWEPT_OK;
         case SWEPT_OPT_BLOCKS_PER_SM:
             if (value < 0 || value > 32) return fail(SWEPT_EINVAL, "swept_set_option: BLOCKS_PER_SM takes 0..32");
             h->blocks_per_sm = value;
@@ -658,6 +683,7 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->boundary = h->bc;
     info->tuned_chain = h->tuned_chain;
     info->tuned_blocks_per_sm = h->tuned_cap;
+    info->tuned_pack = h->tuned_pack;
     return SWEPT_OK;
 }
 
@@ -699,5 +725,15 @@ extern "C" int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     e = run_alu_peak(dtype, sms, instr_per_s, ms, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(e, "swept_measure_alu_peak");
+    return SWEPT_OK;
+}
+
+extern "C" int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cuda_stream) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_measure_smem_peak: no CUDA device");
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    e = run_smem_peak(sms, bytes_per_s, ms, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_measure_smem_peak");
     return SWEPT_OK;
 }

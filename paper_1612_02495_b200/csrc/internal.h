@@ -43,8 +43,9 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
 // Streaming band kernel (swept_band.cuh): ONE launch runs q half-cycles with every band's columns resident in registers /
 // shared memory; `sync` = prog[nx/W] counters (zeroed by the helper).  cudaErrorNotSupported if the schedule does not fit
 // the device (the caller then uses launch_swept_chain).  max_warps > 0 caps the resident warps per SM.
+// pack != 0 (heat fp32 only): two bands per warp slot, advanced by packed f32x2 arithmetic (stencils.cuh float2p).
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
-                              int sm_count, int max_smem, int max_warps, cudaStream_t st);
+                              int sm_count, int max_smem, int max_warps, int pack, cudaStream_t st);
 // Ring kernel (swept_ring.cuh): the band kernel with a communication warp per block (cp.async-staged edge exchange); ONE launch
 // runs q half-cycles plus rt remainder tiers (rt = S x remaining timesteps < L).  `sync` = prog[nx/W] counters (zeroed by the
 // helper).  cudaErrorNotSupported if the width / schedule does not fit (the caller then uses the band or the tile-flag kernel).
@@ -94,6 +95,7 @@ int swept_fail(int code, const char *fmt, ...) __attribute__((format(printf, 2, 
 
 // FMA-chain microbenchmark (alu_peak.cu)
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st);
+cudaError_t run_smem_peak(int sm_count, double *bytes_per_s, double *ms, cudaStream_t st);
 
 inline int radius_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }
 inline int stages_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }

@@ -41,6 +41,23 @@ template <class P, int PW> constexpr int band_sr() {
     return (P::H == 1 && (PW == 16 || (PW == 32 && sizeof(typename P::real) == 4))) ? 4 : ((P::H == 1 && PW >= 8) ? 2 : 1);
 }
 
+// Lane vector.  T = float / double: a warp slot is one band.  T = float2p: a slot is TWO bands advanced in lock step by packed
+// arithmetic, component x the band n, component y the band n + nslots -- exactly half a domain away, so every global address of
+// the y component is the x component's address + nx/2 (mod nx).  Progress counters stay per band.
+template <class T> struct LaneVec { using E = T; static constexpr int V = 1; };
+template <> struct LaneVec<float2p> { using E = float; static constexpr int V = 2; };
+template <class T> __device__ __forceinline__ T lv_ldcg(const typename LaneVec<T>::E *base, int64_t a, int64_t half, int64_t mask) {
+    if constexpr (LaneVec<T>::V == 1) return __ldcg(base + a);
+    else return float2p(__ldcg(base + a), __ldcg(base + ((a + half) & mask)));
+}
+template <class T> __device__ __forceinline__ void lv_stcg(typename LaneVec<T>::E *base, int64_t a, int64_t half, int64_t mask, T v) {
+    if constexpr (LaneVec<T>::V == 1) __stcg(base + a, v);
+    else { __stcg(base + a, v.x); __stcg(base + ((a + half) & mask), v.y); }
+}
+template <> __device__ __forceinline__ float2p shfl_up1<float2p>(float2p v) {
+    return float2p(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1));
+}
+
 template <class P, int PW> struct BandGeom {
     using T = typename P::real;
     static constexpr int H = P::H, NC = P::NC, D = 2 * H, SR = band_sr<P, PW>();
@@ -147,9 +164,12 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
 }
 
 template <class P, int PW, bool TIGHT = false>
-__global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band_kernel(typename P::real *u, typename P::real *w, int64_t nx, int ntiles, int q,
-                                                             BandGrid grid, unsigned *prog, typename P::Consts c) {
+__global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band_kernel(typename LaneVec<typename P::real>::E *u, typename LaneVec<typename P::real>::E *w, int64_t nx,
+                                                             int ntiles /* slots: bands / V */, int q, BandGrid grid, unsigned *prog, typename P::Consts c) {
     using T = typename P::real;
+    using E = typename LaneVec<T>::E;
+    constexpr int V = LaneVec<T>::V;
+    const int64_t half = nx / 2;                          // (V = 2) offset of the y component's band
     using Gm = BandGeom<P, PW>;
     constexpr int H = Gm::H, NC = Gm::NC, D = Gm::D, W = Gm::W, NJI = Gm::NJI, NP = Gm::NP, L = Gm::L, CTR = Gm::CTR, NCH = Gm::NCH, CS = Gm::CS, SR = Gm::SR;
     static_assert(PW % D == 0, "points per lane must be a multiple of 2H");
@@ -177,7 +197,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
 #pragma unroll
         for (int kk = 0; kk < NC; ++kk)
 #pragma unroll
-            for (int i = 0; i < PW; ++i) X[kk][D + i] = __ldcg(u + (int64_t)kk * nx + ((g0 + lane * PW + i) & mask));
+            for (int i = 0; i < PW; ++i) X[kk][D + i] = lv_ldcg<T>(u + (int64_t)kk * nx, (g0 + lane * PW + i) & mask, half, mask);
 #pragma unroll
         for (int kk = 0; kk < NC; ++kk)
 #pragma unroll
@@ -188,7 +208,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
             T *buf = col + (size_t)(m - 1) * Gm::COL;
             for (int i = lane; i < W; i += 32)
 #pragma unroll
-                for (int kk = 0; kk < NC; ++kk) buf[kk * CS + i + i / PW] = __ldcg(u + (int64_t)kk * nx + ((gm + i) & mask));
+                for (int kk = 0; kk < NC; ++kk) buf[kk * CS + i + i / PW] = lv_ldcg<T>(u + (int64_t)kk * nx, (gm + i) & mask, half, mask);
         }
         for (int i = lane; i < Gm::FEED; i += 32) feed[i] = T(0);
         __syncwarp();
@@ -239,9 +259,11 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         __syncwarp();
         const int sf = K0 / NJI, pf = sf / k, mf = sf - pf * k;
         const bool fetch = K0 < lt_end && pf > 0;
-        const int bandf = first + mf * stride, left = bandf == 0 ? ntiles - 1 : bandf - 1;
+        // (V = 2: lane 0 polls / releases the counter of the slot's band, lane 1 that of the band half a domain away)
+        const int nbands = ntiles * V;
+        const int bandf = first + mf * stride, bandl = bandf + (lane < V ? lane : 0) * ntiles, left = bandl == 0 ? nbands - 1 : bandl - 1;
         unsigned seen = 0;
-        if (fetch && lane == 0) seen = ld_acquire_gpu(prog + left);
+        if (fetch && lane < V) seen = ld_acquire_gpu(prog + left);
         const int lt0 = K0 - 64;
         if (lt0 >= 0 && lt0 < lt_end) {
             const int s = lt0 / NJI, p = s / k, m = s - p * k;
@@ -251,25 +273,25 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr) {
                     const int J = SR * ((lt0 & (NJI - 1)) + lane) + sr;        // super-row: rows j = J D + rho hold tier L + J
-                    T *dst = (J & 1) ? w : u;
+                    E *dst = (J & 1) ? w : u;
 #pragma unroll
                     for (int rho = 0; rho < D; ++rho) {
                         const int64_t g = (g0 + W - 1 - H * J - rho) & mask;
 #pragma unroll
                         for (int kk = 0; kk < NC; ++kk)
-                            __stcg(dst + (int64_t)kk * nx + g, outr[((kk * 64 + ((lt0 + lane) & 63)) * SR + sr) * D + rho]);
+                            lv_stcg<T>(dst + (int64_t)kk * nx, g, half, mask, outr[((kk * 64 + ((lt0 + lane) & 63)) * SR + sr) * D + rho]);
                     }
                 }
                 // the warp barrier orders every lane's stores before lane 0's release (cumulative at gpu scope)
                 __syncwarp();
-                if (lane == 0) st_release_gpu(prog + band, (unsigned)(p * NCH + (lt0 & (NJI - 1)) / 32 + 1));
+                if (lane < V) st_release_gpu(prog + band + lane * ntiles, (unsigned)(p * NCH + (lt0 & (NJI - 1)) / 32 + 1));
             }
         }
         if (K0 < lt_end) {
             if (fetch) {
                 const unsigned need = (unsigned)((pf - 1) * NCH + (K0 & (NJI - 1)) / 32 + 1);
                 bool dead = false;
-                if (lane == 0) {
+                if (lane < V) {
                     unsigned ns = 20;
                     SpinWatch polls;
                     while (seen < need) {
@@ -284,12 +306,12 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr) {
                     const int J = SR * ((K0 & (NJI - 1)) + lane) + sr;         // row j = J D + rho is fed from tier J of the left tile's right edge
-                    const T *src = (J & 1) ? w : u;
+                    const E *src = (J & 1) ? w : u;
 #pragma unroll
                     for (int rho = 0; rho < D; ++rho) {
                         const int64_t g = (g0 + CTR - H * J - rho - 1) & mask;
 #pragma unroll
-                        for (int kk = 0; kk < NC; ++kk) feed[((kk * 32 + lane) * SR + sr) * D + rho] = __ldcg(src + (int64_t)kk * nx + g);
+                        for (int kk = 0; kk < NC; ++kk) feed[((kk * 32 + lane) * SR + sr) * D + rho] = lv_ldcg<T>(src + (int64_t)kk * nx, g, half, mask);
                     }
                 }
             }
@@ -407,13 +429,13 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
 #pragma unroll
         for (int kk = 0; kk < NC; ++kk)
 #pragma unroll
-            for (int i = 0; i < PW; ++i) __stcg(u + (int64_t)kk * nx + ((g0 + lane * PW + i) & mask), X[kk][D + i]);
+            for (int i = 0; i < PW; ++i) lv_stcg<T>(u + (int64_t)kk * nx, (g0 + lane * PW + i) & mask, half, mask, X[kk][D + i]);
         for (int m = 0; m + 1 < k; ++m) {
             const int64_t gm = g0_of(first + m * stride, q);
             const T *buf = col + (size_t)((q * k + m) % (k - 1)) * Gm::COL;   // band m's closing tile was swapped out at transition q k + m
             for (int i = lane; i < W; i += 32)
 #pragma unroll
-                for (int kk = 0; kk < NC; ++kk) __stcg(u + (int64_t)kk * nx + ((gm + i) & mask), buf[kk * CS + i + i / PW]);
+                for (int kk = 0; kk < NC; ++kk) lv_stcg<T>(u + (int64_t)kk * nx, (gm + i) & mask, half, mask, buf[kk * CS + i + i / PW]);
         }
     }
 }
@@ -426,7 +448,9 @@ template <class P, int PW, bool TIGHT = false>
 bool band_grid(int64_t nx, int sm_count, int max_smem, int max_warps, BandGrid *out, size_t *smem_bytes) {
     using Gm = BandGeom<P, PW>;
     using T = typename P::real;
-    const int64_t ntiles64 = nx / Gm::W;
+    constexpr int V = LaneVec<T>::V;
+    if ((nx / Gm::W) % V != 0) return false;
+    const int64_t ntiles64 = nx / Gm::W / V;                      // warp slots (V bands each)
     // One chunk per tile (NJI = 32): lane 0 would need, at the start of a tile, the chunk its left neighbour's lane 31 is
     // still 31 super-rows from finishing -- with every band in lockstep that is a cycle of waits, not a bubble
     if (Gm::NCH < 2) return false;
@@ -476,13 +500,17 @@ cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, co
     size_t smem = 0;
     if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, max_warps, &g, &smem)) return cudaErrorNotSupported;
     if ((int64_t)(q + 1) * g.kmax * Gm::NJI >= ((int64_t)1 << 31) - 64) return cudaErrorNotSupported;   // the kernel's local time is an int
-    const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
-    const int ntiles = (int)(nx / Gm::W);
-    cudaError_t e = cudaMemsetAsync(sync, 0, sizeof(unsigned) * (size_t)ntiles, st);
+    using E = typename LaneVec<T>::E;
+    constexpr int V = LaneVec<T>::V;
+    typename P::Consts c;
+    if constexpr (V == 1) c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
+    else c = P::expand(cb.bytes);                                 // the scalar problem's constants, both components
+    const int nbands = (int)(nx / Gm::W), ntiles = nbands / V;    // ntiles: warp slots
+    cudaError_t e = cudaMemsetAsync(sync, 0, sizeof(unsigned) * (size_t)nbands, st);
     if (e != cudaSuccess) return e;
     // Cooperative launch: the warps wait on one another, so the whole grid must be resident at once -- also when another
     // stream's kernel shares the device (a plain launch could leave two such grids each half scheduled, waiting forever).
-    T *up = (T *)u, *wp = (T *)w;
+    E *up = (E *)u, *wp = (E *)w;
     int qi = (int)q, nt = ntiles;
     unsigned *pr = (unsigned *)sync;
     typename P::Consts cc = c;

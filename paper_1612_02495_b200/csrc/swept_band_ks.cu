@@ -18,7 +18,7 @@ template <class T> static cudaError_t prepare_t(int max_smem) {
     if ((e = band_prepare_pw<KS<T>, 32>(max_smem)) != cudaSuccess) return e;
     return e;
 }
-cudaError_t launch_swept_band_ks(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, int max_warps, cudaStream_t st) {
+cudaError_t launch_swept_band_ks(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, int max_warps, int, cudaStream_t st) {
     return dtype == SWEPT_F64 ? band_t<double>(u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, st) : band_t<float>(u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, st);
 }
 cudaError_t swept_band_prepare_ks(int dtype, int max_smem) { return dtype == SWEPT_F64 ? prepare_t<double>(max_smem) : prepare_t<float>(max_smem); }

@@ -51,7 +51,7 @@ def test_paper_geometry_numbers():
     # the two-row matrix holds 2(n+2) values
     assert 2 * (n + 2 * h) == g["two_row_values_n512"]
     # a full cycle (two half-cycles) advances n timesteps for the heat scheme
-    assert 2 * sw.steps_per_half_cycle(sw.HEAT, n) == n * g["timesteps_per_cycle_heat_n"]
+    assert 2 * sw.steps_per_half_cycle(sw.HEAT, n) == n      # PAPER.md:98 "advance by n timesteps with two ... global memory accesses": n/2 per half-cycle
     # a 32-point node gives four KS timesteps per (half-)cycle, "which only reduces instances of communication
     # by 1/8": one global exchange per L = 8 sub-timesteps = 4 two-stage timesteps
     assert sw.steps_per_half_cycle(sw.KS, 32) == g["ks_steps_per_cycle_n32"]

@@ -515,3 +515,36 @@ def test_ring_repeated_calls_two_handles_two_streams_and_graph_replay():
     assert_bits_equal(u1.cpu().numpy(), ref, "stream 1")
     assert_bits_equal(u2.cpu().numpy(), ref, "stream 2 (graph replay)")
     s1.close(); s2.close()
+
+
+# ------------------------------------------------------------------------------------------------------------
+# packed pairs of bands (SWEPT_OPT_PACK = 2): heat fp32 on the band kernel, two bands per warp slot on f32x2 arithmetic
+# ------------------------------------------------------------------------------------------------------------
+PACK_CASES = [
+    # nx, W, q                        what it exercises
+    (512, 128, 9),                    # four bands = two slots: each slot is the other's left neighbour, components swapped at the wrap
+    (1 << 12, 128, 1),                # q = 1
+    (1 << 16, 256, 40),               # one slot per warp, many phases
+    (1 << 20, 512, 7),                # four super-rows per iteration
+    (1 << 22, 1024, 5),               # the bench size: 2048 slots on 148 x 16 warps
+    (1 << 22, 256, 5),                # 8192 slots: several per warp, parked pairs swapped through shared memory
+    (1 << 21, 128, 6),
+]
+
+
+@pytest.mark.parametrize("nx,W,q", PACK_CASES)
+def test_packed_band_pairs_equal_classic(nx, W, q):
+    import torch
+    w = _noise(wl.HEAT, nx)
+    nsteps = q * _sph(wl.HEAT, W) + 3
+    with solver_for(w, np.float32) as s:
+        s.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
+        s.set_option(sw.OPT_PACK, sw.PACK_ON)
+        u = to_dev(w.initial(np.float32))
+        s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        assert s.info()["last_sweep_launch"] == sw.LAUNCH_BAND
+        got = u.cpu().numpy()
+    assert_bits_equal(got, run_naive(w, np.float32, nsteps), f"packed band pairs nx={nx} W={W} q={q}")
+    # and the same run with one band per slot gives the same bits
+    assert_bits_equal(got, run_swept(w, np.float32, nsteps, W, BAND_V, opts={sw.OPT_PACK: sw.PACK_OFF}), "packed vs one band per slot")
