@@ -106,8 +106,9 @@ enum {
  *   DIAMOND  `count` consecutive diamond launches, the first at `offset`, then alternating 0 <-> W/2
  *   DOWN     closing inverted triangles at `offset`
  *   CHAIN    `count` half-cycles (1 UP + (count-1) DIAMOND + 1 DOWN phases, offsets 0, W/2, 0, ...) in ONE launch
- *   BAND     the same in ONE launch of the streaming band kernel (SWEPT_OPT_CHAIN = 2; a handle whose device cannot hold
- *            the band schedule runs the entry as CHAIN)
+ *   BAND     `count` half-cycles AND `offset` remainder timesteps (a truncated closing cycle, as RING) in ONE launch of the
+ *            streaming band kernel (SWEPT_OPT_CHAIN = 2; a handle whose device cannot hold the band schedule runs the same
+ *            timesteps as the plan of SWEPT_OPT_CHAIN = 1)
  *   RING     `count` half-cycles AND `offset` remainder timesteps (offset < L/S; a truncated closing cycle) in ONE launch of
  *            the ring kernel (SWEPT_OPT_CHAIN = 3): the whole swept_run.  A handle whose device cannot hold the schedule runs
  *            the same timesteps as the plan of SWEPT_OPT_CHAIN = 2.                                                   */

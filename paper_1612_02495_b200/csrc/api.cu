@@ -383,9 +383,10 @@ static int64_t build_plan(int problem, int dtype, int64_t nx, int64_t nsteps, in
     const int64_t sph = W / per;
     const int64_t q = nsteps / sph;
     int64_t r = nsteps % sph;
-    // ring kernel (chain = 3): the q half-cycles AND the remainder (as a truncated closing cycle) in one launch; entry.offset = r
-    if (chain == 3 && kernel == SWEPT_KERNEL_WAVE && !bc && nsteps > 0 && swept_ring_supports(problem, W) && nx / W >= 2) {
-        push(SWEPT_LAUNCH_RING, W, r, q);
+    // ring kernel (chain = 3) and band kernel (chain = 2): the q half-cycles AND the remainder (as a truncated closing cycle) in one
+    // launch; entry.offset = r.  (Both need tiles of at least 64 iterations and two tiles.)
+    if (chain >= 2 && kernel == SWEPT_KERNEL_WAVE && !bc && nsteps > 0 && swept_ring_supports(problem, W) && nx / W >= 2) {
+        push(chain == 3 ? SWEPT_LAUNCH_RING : SWEPT_LAUNCH_BAND, W, r, q);
         return n;
     }
     char buf[160];
@@ -475,10 +476,12 @@ static cudaError_t enqueue_swept(swept_ctx *h, int kernel, void *d_u, int64_t ns
             case SWEPT_LAUNCH_BAND:
                 // bands wrap around the periodic domain; a rod with insulated ends runs on the tile-flag kernel
                 e = h->bc ? cudaErrorNotSupported
-                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->sm_count, h->max_smem, 4 * effective_cap(h, L.tile_width), effective_pack(h, L.tile_width), st);
+                          : launch_swept_band(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, (int)(L.offset * h->S), h->sync, h->cb, h->sm_count, h->max_smem, 4 * effective_cap(h, L.tile_width), effective_pack(h, L.tile_width), st);
                 if (e != cudaErrorNotSupported && e != cudaErrorCooperativeLaunchTooLarge) { ++*launches; h->last_sweep_launch = SWEPT_LAUNCH_BAND; break; }
                 cudaGetLastError();
-                /* the band schedule does not fit this device / size: same half-cycles through the tile-flag kernel */
+                // the band schedule does not fit this device / size: with a truncated closing cycle, the same timesteps as remainder
+                // launches + the tile-flag kernel; without, the same half-cycles through the tile-flag kernel
+                if (L.offset > 0 || L.count == 0) return enqueue_swept(h, kernel, d_u, nsteps, W, st, launches, 1);
                 /* fall through */
             case SWEPT_LAUNCH_CHAIN:
                 e = launch_swept_chain(h->problem, h->dtype, d_u, h->work, h->nx, L.tile_width, L.count, h->sync, h->cb, h->warps_per_block,

@@ -58,6 +58,11 @@ template <> __device__ __forceinline__ float2p shfl_up1<float2p>(float2p v) {
     return float2p(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1));
 }
 
+#ifndef STEADY_UNROLL
+#define STEADY_UNROLL 1
+#endif
+constexpr int STEADY_UNROLL_N = STEADY_UNROLL;      // iterations of the steady loop unrolled together
+
 template <class P, int PW> struct BandGeom {
     using T = typename P::real;
     static constexpr int H = P::H, NC = P::NC, D = 2 * H, SR = band_sr<P, PW>();
@@ -165,7 +170,7 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
 
 template <class P, int PW, bool TIGHT = false>
 __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band_kernel(typename LaneVec<typename P::real>::E *u, typename LaneVec<typename P::real>::E *w, int64_t nx,
-                                                             int ntiles /* slots: bands / V */, int q, BandGrid grid, unsigned *prog, typename P::Consts c) {
+                                                             int ntiles /* slots: bands / V */, int q, int rt, BandGrid grid, unsigned *prog, typename P::Consts c) {
     using T = typename P::real;
     using E = typename LaneVec<T>::E;
     constexpr int V = LaneVec<T>::V;
@@ -182,7 +187,10 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
     const int first = band_first(grid, (int)blockIdx.x, warp), stride = band_stride(grid);   // bands first, first + stride, ...
     const int k = band_count(grid, (int)blockIdx.x, warp, ntiles);
     if (k == 0) return;
-    const int n_items = k * (q + 1);
+    // rt > 0: the remainder as a truncated closing cycle (swept_ring.cuh; reading S3'): phase q runs on to tier L + rt and
+    // one more phase q + 1 runs up to tier rt
+    const int nph = q + 1 + (rt > 0 ? 1 : 0);
+    const int n_items = k * nph;
     const int lt_end = n_items * NJI;                     // < 2^31: the host refuses longer runs
 
     T *base = reinterpret_cast<T *>(smem_raw) + (size_t)warp * Gm::warp_values(grid.kmax);
@@ -214,12 +222,12 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         __syncwarp();
     }
 
-    int p_cur = 0, lo = L, hi = 0x7fffffff;              // this lane's tile: phase, and the tiers (lo, hi] it updates
+    int p_cur = 0, lo = L, hi = 0x3fffffff;              // this lane's tile: phase, and the tiers (lo, hi] it updates
     bool interior = false;                               // p_cur is a diamond phase: every point of the tile is updated
     auto set_phase = [&](int s) {
         p_cur = s / k;
         lo = p_cur == 0 ? L : 0;
-        hi = p_cur == q ? L : 0x7fffffff;
+        hi = p_cur < q ? 0x3fffffff : (p_cur == q ? L + rt : rt);
         interior = p_cur > 0 && p_cur < q;
     };
     // This lane enters tile s >= 1 of a warp that owns k > 1 bands: swap its PW columns with the parked copy of the incoming
@@ -267,7 +275,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         const int lt0 = K0 - 64;
         if (lt0 >= 0 && lt0 < lt_end) {
             const int s = lt0 / NJI, p = s / k, m = s - p * k;
-            if (p < q) {
+            if (p < nph - 1) {
                 const int band = first + m * stride;
                 const int64_t g0 = g0_of(band, p);
 #pragma unroll
@@ -335,6 +343,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                 int J = (K0 - lane) & (NJI - 1);
                 const T *fp = feed;
                 T *op = outr + ((K0 - 31) & 63) * SR * D;     // lane 31's slot of local time K0 - 31
+#pragma unroll(STEADY_UNROLL_N)
                 for (int it = 0; it < 32; ++it) {
                     T recv[SR][NC][D];
 #pragma unroll
@@ -411,7 +420,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
             } else if (act) {
                 band_super_rows<P, PW, SR, false>(X, recv, keep, c, tb, lo, hi);
             }
-            if (act && lane == 31 && p_cur < q) {         // the row outputs of the SR super-rows
+            if (act && lane == 31 && p_cur < nph - 1) {   // the row outputs of the SR super-rows
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr)
 #pragma unroll
@@ -423,16 +432,38 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         }
     }
 
-    // ---- closing inverted triangles done: registers hold band k-1's flat values, the parked copies the other bands'
+    // ---- With a truncated closing cycle phase q has a consumer, and its row outputs lie in the span the flat field is stored over:
+    // wait until every warp of the grid is through its last tile (swept_ring.cuh explains the hazard)
+    if (rt > 0) {
+        bool dead = false;
+        __syncwarp();
+        if (lane == 0) {
+            const int stride_all = band_stride(grid);
+            const unsigned total = (unsigned)(ntiles < stride_all ? ntiles : stride_all);
+            __threadfence();
+            atomicAdd(prog + ntiles * V, 1u);
+            unsigned ns = 100;
+            SpinWatch polls;
+            while (ld_acquire_gpu(prog + ntiles * V) < total) {
+                __nanosleep(ns);
+                if (ns < 6400) ns *= 2;
+                if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
+            }
+        }
+        if (__any_sync(0xffffffffu, dead)) return;
+    }
+    // ---- all phases done: column i of a band ended at x = g0(band, q) + i - H rt; registers hold band k-1's flat values, the
+    // parked copies the other bands'
     {
-        const int64_t g0 = g0_of(first + (k - 1) * stride, q);
+        const int64_t sh = (rt > 0 ? W / 2 : 0) - H * rt + nx;   // g0(q) = g0(last phase) + W/2 when the extra phase ran
+        const int64_t g0 = g0_of(first + (k - 1) * stride, nph - 1) + sh;
 #pragma unroll
         for (int kk = 0; kk < NC; ++kk)
 #pragma unroll
             for (int i = 0; i < PW; ++i) lv_stcg<T>(u + (int64_t)kk * nx, (g0 + lane * PW + i) & mask, half, mask, X[kk][D + i]);
         for (int m = 0; m + 1 < k; ++m) {
-            const int64_t gm = g0_of(first + m * stride, q);
-            const T *buf = col + (size_t)((q * k + m) % (k - 1)) * Gm::COL;   // band m's closing tile was swapped out at transition q k + m
+            const int64_t gm = g0_of(first + m * stride, nph - 1) + sh;
+            const T *buf = col + (size_t)(((nph - 1) * k + m) % (k - 1)) * Gm::COL;   // band m's last tile was swapped out at transition (nph-1) k + m
             for (int i = lane; i < W; i += 32)
 #pragma unroll
                 for (int kk = 0; kk < NC; ++kk) lv_stcg<T>(u + (int64_t)kk * nx, (gm + i) & mask, half, mask, buf[kk * CS + i + i / PW]);
@@ -486,7 +517,7 @@ bool band_grid(int64_t nx, int sm_count, int max_smem, int max_warps, BandGrid *
 
 // `sync` = prog[ntiles] (zeroed here).  Returns cudaErrorNotSupported when the band schedule does not fit.
 template <class P, int PW, bool TIGHT = false>
-cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, const ConstBlock &cb, int sm_count, int max_smem, int max_warps,
+cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, int rt, void *sync, const ConstBlock &cb, int sm_count, int max_smem, int max_warps,
                          cudaStream_t st) {
     using T = typename P::real;
     using Gm = BandGeom<P, PW>;
@@ -494,27 +525,28 @@ cudaError_t wave_band_pw(void *u, void *w, int64_t nx, int64_t q, void *sync, co
         // more bands than the roomy build has warps, and no more than the tight build has (one band per warp: its spills make
         // the band swaps of k > 1 slower than the roomy build's)
         if (nx / Gm::W > (int64_t)sm_count * (band_max_threads<P, PW, false>() / 32) && nx / Gm::W <= (int64_t)sm_count * (band_max_threads<P, PW, true>() / 32))
-            return wave_band_pw<P, PW, true>(u, w, nx, q, sync, cb, sm_count, max_smem, max_warps, st);
+            return wave_band_pw<P, PW, true>(u, w, nx, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
     }
     BandGrid g;
     size_t smem = 0;
-    if (q < 1 || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, max_warps, &g, &smem)) return cudaErrorNotSupported;
-    if ((int64_t)(q + 1) * g.kmax * Gm::NJI >= ((int64_t)1 << 31) - 64) return cudaErrorNotSupported;   // the kernel's local time is an int
+    if (q < 0 || (q == 0 && rt == 0) || rt < 0 || rt >= Gm::L || q > (1 << 24) / Gm::NCH || !band_grid<P, PW, TIGHT>(nx, sm_count, max_smem, max_warps, &g, &smem))
+        return cudaErrorNotSupported;
+    if ((int64_t)(q + 2) * g.kmax * Gm::NJI >= ((int64_t)1 << 30)) return cudaErrorNotSupported;   // the kernel's local time is an int
     using E = typename LaneVec<T>::E;
     constexpr int V = LaneVec<T>::V;
     typename P::Consts c;
     if constexpr (V == 1) c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
     else c = P::expand(cb.bytes);                                 // the scalar problem's constants, both components
     const int nbands = (int)(nx / Gm::W), ntiles = nbands / V;    // ntiles: warp slots
-    cudaError_t e = cudaMemsetAsync(sync, 0, sizeof(unsigned) * (size_t)nbands, st);
+    cudaError_t e = cudaMemsetAsync(sync, 0, sizeof(unsigned) * (size_t)(nbands + 1), st);   // prog[nbands] + the end-of-run arrival count
     if (e != cudaSuccess) return e;
     // Cooperative launch: the warps wait on one another, so the whole grid must be resident at once -- also when another
     // stream's kernel shares the device (a plain launch could leave two such grids each half scheduled, waiting forever).
     E *up = (E *)u, *wp = (E *)w;
-    int qi = (int)q, nt = ntiles;
+    int qi = (int)q, nt = ntiles, rti = rt;
     unsigned *pr = (unsigned *)sync;
     typename P::Consts cc = c;
-    void *args[] = {&up, &wp, &nx, &nt, &qi, &g, &pr, &cc};
+    void *args[] = {&up, &wp, &nx, &nt, &qi, &rti, &g, &pr, &cc};
     return cudaLaunchCooperativeKernel((const void *)swept_band_kernel<P, PW, TIGHT>, dim3((unsigned)g.nblocks), dim3((unsigned)(g.wpb * 32)), args, smem, st);
 }
 

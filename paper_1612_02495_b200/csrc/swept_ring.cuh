@@ -393,7 +393,7 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
                 constexpr bool SWAP = decltype(swap_tag)::value;
                 int J = (K0 - lane) & (NJI - 1);
                 int fs = K0 & (CAP - 1), os = (K0 - 31) & (OCAP - 1);     // ring slots: lane 0's local time K0, lane 31's K0 - 31
-#pragma unroll 1
+#pragma unroll(STEADY_UNROLL_N)
                 for (int it = 0; it < CH; ++it) {
                     const T *fp = feed + fs * SR * D;
                     T recv[SR][NC][D];

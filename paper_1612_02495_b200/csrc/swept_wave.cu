@@ -9,7 +9,7 @@ namespace swept {
     cudaError_t launch_swept_chain_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                \
                                           const ConstBlock &cb, int wpb, size_t smem_floor, int sm_count, int bc, cudaStream_t st); \
     cudaError_t swept_wave_prepare_##prob(int dtype, int max_smem);                                                             \
-    cudaError_t launch_swept_band_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync,                 \
+    cudaError_t launch_swept_band_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync,         \
                                          const ConstBlock &cb, int sm_count, int max_smem, int max_warps, int pack, cudaStream_t st); \
     cudaError_t swept_band_prepare_##prob(int dtype, int max_smem);                                                             \
     cudaError_t launch_swept_ring_##prob(int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync,         \
@@ -47,11 +47,11 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
     return launch_swept_chain_euler(dtype, u, w, nx, W, q, sync, cb, warps_per_block, floor, sm_count, bc, st);
 }
 
-cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, void *sync, const ConstBlock &cb,
+cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,
                               int sm_count, int max_smem, int max_warps, int pack, cudaStream_t st) {
-    if (problem == SWEPT_HEAT) return launch_swept_band_heat(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, pack, st);
-    if (problem == SWEPT_KS) return launch_swept_band_ks(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, 0, st);
-    return launch_swept_band_euler(dtype, u, w, nx, W, q, sync, cb, sm_count, max_smem, max_warps, 0, st);
+    if (problem == SWEPT_HEAT) return launch_swept_band_heat(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, pack, st);
+    if (problem == SWEPT_KS) return launch_swept_band_ks(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, 0, st);
+    return launch_swept_band_euler(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, 0, st);
 }
 
 cudaError_t launch_swept_ring(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,

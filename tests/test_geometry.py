@@ -178,11 +178,11 @@ class Model:
             elif kind == sw.LAUNCH_DIAMOND:
                 for k in range(count):
                     self.launch("diamond", W, offset if k % 2 == 0 else (0 if offset else W // 2))
+            elif kind == sw.LAUNCH_RING or (kind == sw.LAUNCH_BAND and (offset or not count)):
+                self.ring(W, count, offset)                      # the whole run in one launch, remainder as a truncated closing cycle
             elif kind in (sw.LAUNCH_CHAIN, sw.LAUNCH_BAND):      # the same phases in one launch (tile flags / streaming bands)
                 for p in range(count + 1):
                     self.launch("up" if p == 0 else ("down" if p == count else "diamond"), W, W // 2 if p & 1 else 0)
-            elif kind == sw.LAUNCH_RING:
-                self.ring(W, count, offset)
             else:
                 raise AssertionError(kind)
 
@@ -227,10 +227,9 @@ def test_plan_structure_and_launch_counts():
     assert [(k, W) for k, W, _, _ in plan] == [(sw.LAUNCH_UP, 512), (sw.LAUNCH_DOWN, 512), (sw.LAUNCH_UP, 128), (sw.LAUNCH_DOWN, 128),
                                                (sw.LAUNCH_CLASSIC, 0), (sw.LAUNCH_CHAIN, 1024)]
     assert plan[-1][3] == 97 and plan[-2][3] == 16
-    # SWEPT_OPT_CHAIN = 2 (streaming bands) differs only in the kind of the last entry
-    band = sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE, chain=sw.CHAIN_BANDS)
-    assert band[:-1] == plan[:-1] and band[-1] == (sw.LAUNCH_BAND, 1024, 0, 97)
-    # the default (SWEPT_OPT_CHAIN = 3, ring kernel): ONE launch, the 336 remainder timesteps as a truncated closing cycle
+    # SWEPT_OPT_CHAIN = 2 (streaming bands) and the default 3 (ring kernel): ONE launch, the 336 remainder timesteps as a
+    # truncated closing cycle inside it
+    assert sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE, chain=sw.CHAIN_BANDS) == [(sw.LAUNCH_BAND, 1024, 336, 97)]
     assert sw.plan(sw.HEAT, 1 << 22, 50000, 1024, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_RING, 1024, 336, 97)]
     assert sw.plan(sw.KS, 4096, 3, 256, kernel=sw.KERNEL_WAVE) == [(sw.LAUNCH_RING, 256, 3, 0)]           # q = 0: only the truncated cycle
     # widths the ring kernel does not take (a tile shorter than 64 iterations; a single tile): the plan of option 2

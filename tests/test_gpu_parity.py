@@ -548,3 +548,29 @@ def test_packed_band_pairs_equal_classic(nx, W, q):
     assert_bits_equal(got, run_naive(w, np.float32, nsteps), f"packed band pairs nx={nx} W={W} q={q}")
     # and the same run with one band per slot gives the same bits
     assert_bits_equal(got, run_swept(w, np.float32, nsteps, W, BAND_V, opts={sw.OPT_PACK: sw.PACK_OFF}), "packed vs one band per slot")
+
+
+@pytest.mark.parametrize("problem,dtype,nx,W,q,r,pack", [
+    (wl.HEAT, np.float64, 1 << 11, 128, 5, 37, 0),       # odd remainder
+    (wl.HEAT, np.float64, 1 << 12, 128, 0, 63, 0),       # q = 0: only the truncated cycle, remainder L - 1
+    (wl.HEAT, np.float64, 1 << 22, 1024, 3, 336, 0),     # the bench shape: 1 or 2 bands per warp
+    (wl.HEAT, np.float32, 1 << 22, 1024, 3, 335, 2),     # packed pairs, odd remainder
+    (wl.HEAT, np.float32, 1 << 21, 128, 4, 11, 2),       # packed pairs, several slots per warp
+    (wl.KS, np.float64, 1 << 20, 512, 3, 63, 0),
+    (wl.EULER, np.float64, 1 << 18, 256, 2, 17, 0),
+])
+def test_band_kernel_runs_the_remainder_as_a_truncated_closing_cycle(problem, dtype, nx, W, q, r, pack):
+    import torch
+    w = _noise(problem, nx)
+    nsteps = q * _sph(problem, W) + r
+    with solver_for(w, dtype) as s:
+        s.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
+        if pack:
+            s.set_option(sw.OPT_PACK, pack)
+        u = to_dev(w.initial(dtype))
+        s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        info = s.info()
+        assert info["last_sweep_launch"] == sw.LAUNCH_BAND and info["launches_last_call"] == 1
+        got = u.cpu().numpy()
+    assert_bits_equal(got, run_naive(w, dtype, nsteps), f"band, truncated cycle nx={nx} W={W} q={q} r={r}")
