@@ -266,7 +266,9 @@ def test_mutants_of_the_oracle_fail_the_second_order_pins(name, tmp_path):
     src = open(os.path.join(obuild.HERE, "schemes.inc")).read()
     assert src.count(old) == 1, f"mutation site not found exactly once: {old!r}"
     (tmp_path / "schemes.inc").write_text(src.replace(old, new))
-    shutil.copy(os.path.join(obuild.HERE, "swept_oracle.c"), tmp_path / "swept_oracle.c")
+    for f in os.listdir(obuild.HERE):          # every other source of the oracle library, unchanged
+        if f.endswith((".c", ".inc", ".h")) and f != "schemes.inc":
+            shutil.copy(os.path.join(obuild.HERE, f), tmp_path / f)
     so = tmp_path / "libmutant.so"
     subprocess.run(["gcc", *obuild.CFLAGS, "-o", str(so), "swept_oracle.c", "-lm"], check=True, cwd=tmp_path)
     L = ctypes.CDLL(str(so))
