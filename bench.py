@@ -439,10 +439,12 @@ def run_heat2d(args):
     with sw.Solver2D(n, n, dx, dt, dtype=sw.F64 if args.dtype == "f64" else sw.F32) as s:
         t = timed(lambda: s.naive_run(u, nsteps))
         res["classic"] = n * n * nsteps / t / 1e9
-        for W in (32, 16, 8):
+        for W, kern, kname in ((32, sw.KERNEL2D_WARP, "register kernel"), (32, sw.KERNEL2D_SMEM, "paper-style smem kernel"), (16, sw.KERNEL2D_SMEM, "paper-style smem kernel"),
+                               (8, sw.KERNEL2D_SMEM, "paper-style smem kernel")):
+            s.set_option(sw.OPT2D_KERNEL, kern)
             u.copy_(u0)
             t = timed(lambda: s.swept_run(u, nsteps, W))
-            res[f"swept W={W}"] = n * n * nsteps / t / 1e9
+            res[f"swept W={W} ({kname})"] = n * n * nsteps / t / 1e9
     try:
         hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
     except Exception:

@@ -56,6 +56,15 @@ int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int tile_width, v
 /* The classic decomposition: one kernel per timestep over all nx*ny points, ping-pong with the workspace. */
 int naive2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
 
+/* SWEPT2D_OPT_KERNEL: which kernels run tiles of W = 32 (W = 8, 16 always run on the shared-memory kernels).
+ *   SWEPT2D_KERNEL_WARP (default)  one warp per tile, both planes of the tile in registers, E/W neighbours by shuffle, no barrier
+ *   SWEPT2D_KERNEL_SMEM            the paper's design in 2-D (Fig. 5): block = tile, thread = point, two shared-memory planes
+ * Same regions, tier order and store rule: the two are interchangeable launch by launch and bit-identical.  Errors: SWEPT_EINVAL. */
+#define SWEPT2D_OPT_KERNEL 0
+#define SWEPT2D_KERNEL_WARP 0
+#define SWEPT2D_KERNEL_SMEM 1
+int swept2d_set_option(swept2d_handle_t h, int option, int value);
+
 int swept2d_get_info(swept2d_handle_t h, swept2d_info_t *info);
 int swept2d_destroy(swept2d_handle_t h);
 

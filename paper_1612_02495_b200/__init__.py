@@ -23,6 +23,7 @@ PACK_AUTO, PACK_OFF, PACK_ON = 0, 1, 2
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}
 BC_PERIODIC, BC_INSULATED = 0, 1
+OPT2D_KERNEL, KERNEL2D_WARP, KERNEL2D_SMEM = 0, 0, 1                 # include/swept2d.h: swept2d_set_option
 CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS, CHAIN_RING = 0, 1, 2, 3     # values of OPT_CHAIN (include/swept1d.h); CHAIN_RING is the default
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
@@ -33,7 +34,7 @@ SYMBOLS = (
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
     "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak",
     # include/swept2d.h
-    "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_get_info", "swept2d_destroy",
+    "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -116,6 +117,7 @@ def lib() -> ctypes.CDLL:
     L.swept2d_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, ctypes.POINTER(_Params2D)]
     L.swept2d_run.argtypes = [vp, vp, i64, ci, vp]
     L.naive2d_run.argtypes = [vp, vp, i64, vp]
+    L.swept2d_set_option.argtypes = [vp, ci, ci]
     L.swept2d_get_info.argtypes = [vp, ctypes.POINTER(_Info2D)]
     L.swept2d_destroy.argtypes = [vp]
     for name in SYMBOLS:
@@ -266,6 +268,9 @@ class Solver2D:
 
     def naive_run(self, u, nsteps: int, stream=None) -> None:
         _check(lib().naive2d_run(self._h, self._ptr(u), int(nsteps), _stream_ptr(stream)))
+
+    def set_option(self, option: int, value: int) -> None:
+        _check(lib().swept2d_set_option(self._h, int(option), int(value)))
 
     def info(self) -> dict:
         i = _Info2D()

@@ -21,7 +21,7 @@
 using namespace swept;
 
 struct swept2d_ctx {
-    int dtype, device;
+    int dtype, device, kernel;
     int64_t nx, ny;
     double dx, dt, alpha;
     ConstBlock cb;
@@ -99,6 +99,131 @@ __global__ void __launch_bounds__(W *W) swept2d_kernel(T *__restrict__ p0, T *__
     }
 }
 
+// ---- register-resident tiles (W = 32): one WARP per tile, lane = x, the tile's 32 rows of both planes in registers -----------
+// The paper-style kernel above keeps at most a third (octahedra) or a sixth (bridges) of a block's threads busy and pays a block
+// barrier per tier.  Here a warp owns a 32 x 32 tile: lane x holds column x of plane 0 (newest even tier) and plane 1 (newest odd
+// tier) in a0[32], a1[32]; the N/S neighbours of a point are registers of the same lane, the E/W neighbours two shuffles.  A tier
+// updates the rows [ya, yb) of its rectangle (a warp-uniform branch per row, so rows outside cost nothing) on the lanes [xa, xb)
+// (a predicate).  No shared-memory planes, no barrier: the 1-D register wavefront's idea (swept_wave.cuh) in its 2-D form.
+// Halo: a rectangle reads one point beyond itself, and only the last tier of an inverted pyramid (s = L, the full tile) reaches
+// beyond the tile: rows -1 and W come in two registers per lane, columns -1 and W through 2 x 32 values of shared memory per warp.
+// Same regions, same tier order, same store rule as swept2d_kernel, so the two interoperate and are both bit-identical to the
+// classic path.
+constexpr int WARPS2D = 8;
+
+template <class T, bool SRC0, bool HALO>
+__device__ __forceinline__ void tier32(T (&a0)[32], T (&a1)[32], const int lane, const int xa, const int xb, const int ya, const int yb, const T hS, const T hN,
+                                       const T *hl, const T *hr, const typename Heat2D<T>::Consts &c) {
+    T(&src)[32] = SRC0 ? a0 : a1;
+    T(&dst)[32] = SRC0 ? a1 : a0;
+    const bool act = lane >= xa && lane < xb;
+    // Rows in groups of RG: one warp-uniform branch per group, so that the group's 2 RG shuffles and RG dependent chains
+    // (shuffle -> 2 adds -> add -> fma) overlap -- with a branch per row every chain ran exposed (ncu: `wait` 3.3 per issue, FP64 pipe
+    // 10 %); rows of a group outside [ya, yb) are computed and dropped (3 rows per tier on average).
+    constexpr int RG = 4;
+#pragma unroll
+    for (int g = 0; g < 32 / RG; ++g) {
+        if (RG * g + RG > ya && RG * g < yb) {            // warp-uniform
+            T e[RG], w[RG], v[RG];
+#pragma unroll
+            for (int r = 0; r < RG; ++r) {
+                const int y = RG * g + r;
+                e[r] = __shfl_down_sync(0xffffffffu, src[y], 1);
+                w[r] = __shfl_up_sync(0xffffffffu, src[y], 1);
+                if (HALO) {
+                    if (lane == 0) w[r] = hl[y];
+                    if (lane == 31) e[r] = hr[y];
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < RG; ++r) {
+                const int y = RG * g + r;
+                const T n = y < 31 ? src[y < 31 ? y + 1 : 31] : hN, so = y > 0 ? src[y > 0 ? y - 1 : 0] : hS;
+                v[r] = Heat2D<T>::point(c, src[y], e[r], w[r], n, so);
+            }
+#pragma unroll
+            for (int r = 0; r < RG; ++r) {
+                const int y = RG * g + r;
+                if (act && y >= ya && y < yb) dst[y] = v[r];
+            }
+        }
+    }
+}
+
+// Tiles of origin (ox, oy) + (tile index) * 32; REGION = R_BRIDGES: tiles [0, ntiles) are the x-bridges at origin (ox, oy), tiles
+// [ntiles, 2 ntiles) the y-bridges at origin (oy, ox).
+template <class T, int REGION>
+__global__ void __launch_bounds__(32 * WARPS2D) swept2d_warp_kernel(T *__restrict__ p0, T *__restrict__ p1, int64_t nx, int64_t ny, int ox, int oy, int tiles_x, int64_t ntiles,
+                                                                     typename Heat2D<T>::Consts c) {
+    constexpr int W = 32, L = 16, C = 16;
+    constexpr bool HALO_REGION = REGION == R_INVERTED || REGION == R_OCTAHEDRON;
+    __shared__ T halo[WARPS2D][2][32];
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    int64_t t = (int64_t)blockIdx.x * WARPS2D + warp;
+    if (t >= ntiles * (REGION == R_BRIDGES ? 2 : 1)) return;
+    const bool ybridge = REGION == R_BRIDGES && t >= ntiles;
+    if (ybridge) t -= ntiles;
+    const int64_t gx0 = (t % tiles_x) * W + (ybridge ? oy : ox), gy0 = (t / tiles_x) * W + (ybridge ? ox : oy);
+    const int64_t mx = nx - 1, my = ny - 1;
+    auto gidx = [&](int lx, int ly) -> int64_t { return ((gy0 + ly) & my) * nx + ((gx0 + lx) & mx); };
+    T a0[32], a1[32];
+#pragma unroll
+    for (int y = 0; y < 32; ++y) {
+        const int64_t g = gidx(lane, y);
+        a0[y] = p0[g];
+        a1[y] = REGION != R_PYRAMID ? p1[g] : T(0);
+    }
+    T hS = T(0), hN = T(0);
+    const T *hl = halo[warp][0], *hr = halo[warp][1];
+    if (HALO_REGION) {                                    // tier L reads plane (L - 1) & 1 = 1 one point beyond the tile
+        hS = p1[gidx(lane, -1)];
+        hN = p1[gidx(lane, W)];
+        halo[warp][0][lane] = p1[gidx(-1, lane)];
+        halo[warp][1][lane] = p1[gidx(W, lane)];
+        __syncwarp();
+    }
+    constexpr int S1 = REGION == R_OCTAHEDRON ? 2 * L - 1 : (REGION == R_INVERTED ? L : L - 1);   // (a bridge's tier L is empty)
+    auto rect = [&](int s, int &xa, int &xb, int &ya, int &yb) {
+        if (REGION == R_PYRAMID) { xa = ya = s; xb = yb = W - s; }
+        else if (REGION == R_BRIDGES) {
+            const int ea = C - s, eb = C + s, sa = s, sb = W - s;
+            xa = ybridge ? sa : ea; xb = ybridge ? sb : eb;
+            ya = ybridge ? ea : sa; yb = ybridge ? eb : sb;
+        } else if (s <= L) { xa = ya = C - s; xb = yb = C + s; }
+        else { xa = ya = s - L; xb = yb = W - (s - L); }
+    };
+#pragma unroll 1
+    for (int s = 1; s <= S1; s += 2) {
+        int xa, xb, ya, yb;
+        rect(s, xa, xb, ya, yb);
+        tier32<T, true, false>(a0, a1, lane, xa, xb, ya, yb, hS, hN, hl, hr, c);
+        if (s + 1 <= S1) {
+            rect(s + 1, xa, xb, ya, yb);
+            if (HALO_REGION && s + 1 == L) tier32<T, false, true>(a0, a1, lane, xa, xb, ya, yb, hS, hN, hl, hr, c);
+            else tier32<T, false, false>(a0, a1, lane, xa, xb, ya, yb, hS, hN, hl, hr, c);
+        }
+    }
+    // ---- store what this lane updated: point (x, y) was updated at the tiers [s_lo, s_hi] (closed forms of the rectangles above);
+    // the newest tier goes to its plane, the one before it -- if the point was updated twice or more -- to the other
+    const int x = lane, ux = x < W - 1 - x ? x : W - 1 - x, dx = C - x > x - C + 1 ? C - x : x - C + 1;
+#pragma unroll
+    for (int y = 0; y < 32; ++y) {
+        const int uy = y < W - 1 - y ? y : W - 1 - y, dy = C - y > y - C + 1 ? C - y : y - C + 1;
+        const int umin = ux < uy ? ux : uy, dmax = dx > dy ? dx : dy;
+        int s_lo, s_hi;
+        if (REGION == R_PYRAMID) { s_lo = 1; s_hi = umin; }
+        else if (REGION == R_BRIDGES) { s_lo = ybridge ? dy : dx; s_hi = ybridge ? ux : uy; }
+        else if (REGION == R_INVERTED) { s_lo = dmax; s_hi = L; }
+        else { s_lo = dmax; s_hi = L + umin; }
+        if (s_hi >= s_lo && s_hi >= 1) {
+            const int64_t g = gidx(x, y);
+            const bool odd = (s_hi & 1) != 0;
+            (odd ? p1 : p0)[g] = odd ? a1[y] : a0[y];
+            if (s_hi > s_lo) (odd ? p0 : p1)[g] = odd ? a0[y] : a1[y];
+        }
+    }
+}
+
 template <class T> typename Heat2D<T>::Consts consts_of(const swept2d_ctx *h) { return *reinterpret_cast<const typename Heat2D<T>::Consts *>(h->cb.bytes); }
 
 template <class T> cudaError_t classic2d(swept2d_ctx *h, void *d_u, int64_t nsteps, cudaStream_t st, int64_t *launches) {
@@ -131,7 +256,28 @@ template <class T, int W> cudaError_t sweep2d(swept2d_ctx *h, void *d_u, int64_t
     return cudaGetLastError();
 }
 
+template <class T> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K, cudaStream_t st, int64_t *launches) {
+    if (K <= 0) return cudaSuccess;
+    constexpr int W = 32;
+    T *p0 = (T *)d_u, *p1 = (T *)h->work;
+    const int tiles_x = (int)(h->nx / W);
+    const int64_t ntiles = (h->nx / W) * (h->ny / W);
+    const dim3 block(32 * WARPS2D), grid((unsigned)((ntiles + WARPS2D - 1) / WARPS2D)), grid2((unsigned)((2 * ntiles + WARPS2D - 1) / WARPS2D));
+    const typename Heat2D<T>::Consts c = consts_of<T>(h);
+    swept2d_warp_kernel<T, R_PYRAMID><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, 0, 0, tiles_x, ntiles, c);
+    ++*launches;
+    for (int64_t k = 0; k < K; ++k) {
+        const int a = (int)(k & 1) * (W / 2), b = W / 2 - a;      // a: the alignment that shrinks in this half-cycle
+        swept2d_warp_kernel<T, R_BRIDGES><<<grid2, block, 0, st>>>(p0, p1, h->nx, h->ny, b, a, tiles_x, ntiles, c);
+        if (k == K - 1) swept2d_warp_kernel<T, R_INVERTED><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
+        else swept2d_warp_kernel<T, R_OCTAHEDRON><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
+        *launches += 2;
+    }
+    return cudaGetLastError();
+}
+
 template <class T> cudaError_t sweep2d_w(swept2d_ctx *h, void *d_u, int W, int64_t K, cudaStream_t st, int64_t *launches) {
+    if (W == 32 && h->kernel != SWEPT2D_KERNEL_SMEM) return sweep2d_warp<T>(h, d_u, K, st, launches);
     switch (W) {
         case 8: return sweep2d<T, 8>(h, d_u, K, st, launches);
         case 16: return sweep2d<T, 16>(h, d_u, K, st, launches);
@@ -159,7 +305,7 @@ extern "C" int swept2d_create(swept2d_handle_t *out, int64_t nx, int64_t ny, dou
     if (e != cudaSuccess) { cudaGetLastError(); return swept_fail(SWEPT_ECUDA, "swept2d_create: no CUDA device (this library has no CPU fallback): %s", cudaGetErrorString(e)); }
     swept2d_ctx *h = new (std::nothrow) swept2d_ctx();
     if (!h) return swept_fail(SWEPT_ENOMEM, "swept2d_create: out of host memory");
-    h->dtype = dtype; h->device = dev; h->nx = nx; h->ny = ny; h->dx = dx; h->dt = dt; h->alpha = alpha;
+    h->dtype = dtype; h->device = dev; h->kernel = SWEPT2D_KERNEL_WARP; h->nx = nx; h->ny = ny; h->dx = dx; h->dt = dt; h->alpha = alpha;
     h->launches_last = h->launches_total = 0;
     const double Fo = alpha * dt / (dx * dx);                     // row A0: constants on the host in double, cast once
     memset(h->cb.bytes, 0, sizeof h->cb.bytes);
@@ -213,6 +359,14 @@ extern "C" int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int ti
     if (e != cudaSuccess) { cudaGetLastError(); return swept_fail(SWEPT_ECUDA, "swept2d_run: %s", cudaGetErrorString(e)); }
     h->launches_last = launches;
     h->launches_total += launches;
+    return SWEPT_OK;
+}
+
+extern "C" int swept2d_set_option(swept2d_handle_t h, int option, int value) {
+    if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_set_option: NULL handle");
+    if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM))
+        return swept_fail(SWEPT_EINVAL, "swept2d_set_option: unknown option %d or value %d", option, value);
+    h->kernel = value;
     return SWEPT_OK;
 }
 

@@ -103,6 +103,16 @@ template <class P, int PW, bool TIGHT = false> constexpr int band_max_threads() 
 // super-row s, which super-row s+1 overwrites (the caller shuffles them to lane l+1 next iteration).  tb = tier of the
 // lane's first point in super-row 0; a point of tier t is updated iff lo < t <= hi (ALL: every point -- the diamond
 // phases' steady state, no tier tests, no selects).
+// s / k for 0 <= s, s k < 2^32 without the integer-division sequence (the quotient of a multiply-high by ceil(2^32 / k) is exact
+// in that range); k = 1 -- every grid with no more bands than warps -- costs nothing.  The chunk boundaries divide local tile
+// numbers by the warp's band count several times each: ncu (heat fp64, nx = 2^12) put three MUFU.RCP division sequences per boundary.
+struct DivK {
+    unsigned m;
+    int k;
+    __device__ __forceinline__ explicit DivK(int kk) : m(kk > 1 ? (unsigned)((0x100000000ull + (unsigned)kk - 1) / (unsigned)kk) : 0u), k(kk) {}
+    __device__ __forceinline__ int operator()(int s) const { return k > 1 ? (int)__umulhi((unsigned)s, m) : s; }
+};
+
 template <class P, int PW, int SR, bool ALL>
 __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 * P::H + PW], const typename P::real (&recv)[SR][P::NC][2 * P::H],
                                                 typename P::real (&keep)[SR][P::NC][2 * P::H], const typename P::Consts &c, const int tb,
@@ -222,10 +232,11 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         __syncwarp();
     }
 
+    const DivK divk(k);
     int p_cur = 0, lo = L, hi = 0x3fffffff;              // this lane's tile: phase, and the tiers (lo, hi] it updates
     bool interior = false;                               // p_cur is a diamond phase: every point of the tile is updated
     auto set_phase = [&](int s) {
-        p_cur = s / k;
+        p_cur = divk(s);
         lo = p_cur == 0 ? L : 0;
         hi = p_cur < q ? 0x3fffffff : (p_cur == q ? L + rt : rt);
         interior = p_cur > 0 && p_cur < q;
@@ -265,7 +276,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         // about to fetch, so that its round trip to L2 overlaps the flush below; (1) flush the row outputs lane 31 produced for
         // local times [K0-64, K0-32); (2) fetch the row feed of lane 0 for local times [K0, K0+32).
         __syncwarp();
-        const int sf = K0 / NJI, pf = sf / k, mf = sf - pf * k;
+        const int sf = K0 / NJI, pf = divk(sf), mf = sf - pf * k;
         const bool fetch = K0 < lt_end && pf > 0;
         // (V = 2: lane 0 polls / releases the counter of the slot's band, lane 1 that of the band half a domain away)
         const int nbands = ntiles * V;
@@ -274,7 +285,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         if (fetch && lane < V) seen = ld_acquire_gpu(prog + left);
         const int lt0 = K0 - 64;
         if (lt0 >= 0 && lt0 < lt_end) {
-            const int s = lt0 / NJI, p = s / k, m = s - p * k;
+            const int s = lt0 / NJI, p = divk(s), m = s - p * k;
             if (p < nph - 1) {
                 const int band = first + m * stride;
                 const int64_t g0 = g0_of(band, p);
@@ -332,12 +343,13 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
         bool steady = K0 >= 31 && K0 + 31 < lt_end;
         const bool swapchunk = k > 1 && (K0 & (NJI - 1)) == 0;
         if (steady) {
-            const int pa = ((K0 - 31) / NJI) / k, pb = ((K0 + 31) / NJI) / k;
+            const int pa = divk((K0 - 31) / NJI), pb = divk((K0 + 31) / NJI);
             steady = pa > 0 && pb < q;
         }
         if (steady) {
             // two instances of the loop: the chunk in which lanes swap bands carries the swap and a warp barrier per iteration,
             // the others (7 of 8 at W = 1024) stay free of both
+            constexpr bool ONE_LOOP = P::GROUPED;
             auto steady_chunk = [&](auto swap_tag) {
                 constexpr bool SWAP = decltype(swap_tag)::value;
                 int J = (K0 - lane) & (NJI - 1);
@@ -356,7 +368,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                                 const T r = shfl_up1(keep[sr][kk][rho]);
                                 recv[sr][kk][rho] = lane == 0 ? f : r;
                             }
-                    if (SWAP && J == 0) swap_bands((K0 + it - lane) / NJI);
+                    if (SWAP && (!ONE_LOOP || swapchunk) && J == 0) swap_bands((K0 + it - lane) / NJI);
                     band_super_rows<P, PW, SR, true>(X, recv, keep, c, lane * NP + SR * J + 1, 0, 0);
                     if (lane == 31) {
 #pragma unroll
@@ -370,10 +382,12 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                     fp += SR * D;
                     op += SR * D;
                     if (op == outr + 64 * SR * D) op = outr;
-                    if (SWAP) __syncwarp();               // lane l+1 reads the hand-over slot lane l wrote this iteration
+                    if (SWAP && (!ONE_LOOP || swapchunk)) __syncwarp();   // lane l+1 reads the hand-over slot lane l wrote this iteration
                 }
             };
-            if (swapchunk) steady_chunk(std::true_type{});
+            // Euler's loop body is 40 KB of code: two instances of it, taken in turn by a warp with k > 1 bands, thrash the instruction
+            // cache (ncu, fp64, nx = 2^20: `no_instruction` the top stall, 28 % of the samples) -- one instance, the swap a run-time flag
+            if (ONE_LOOP || swapchunk) steady_chunk(std::true_type{});
             else steady_chunk(std::false_type{});
             continue;
         }

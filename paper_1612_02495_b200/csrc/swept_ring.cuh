@@ -82,6 +82,9 @@ constexpr int RING_ROOMY = 3;
 template <class P, int PW> constexpr int ring_nwmax() {
     const int est = P::NC * (2 * P::H + PW) * (int)(sizeof(typename P::real) / 4) + (P::GROUPED ? 110 : 56 + 16 * (P::H - 1));
     int warps = 65536 / (32 * est);
+#ifdef RING_EXP_EULER_NW
+    if (P::GROUPED && sizeof(typename P::real) == 8 && PW == 8) warps = RING_EXP_EULER_NW;
+#endif
     if (P::H == 2 && !P::GROUPED && sizeof(typename P::real) == 8 && PW == 32) warps = 8;   // KS fp64, 32 points per lane: spills below ~200 registers
     warps = warps >= 4 ? (warps & ~3) : 4;
     return (warps > 28 ? 28 : warps) - 1;
@@ -160,6 +163,7 @@ __device__ __forceinline__ void ring_comm_warp(typename P::real *u, typename P::
     const int first = mine ? band_first(grid, (int)blockIdx.x, lane) : 0;
     const int k = mine ? band_count(grid, (int)blockIdx.x, lane, ntiles) : 0;
     const int lt_end = k * nph * NJI;
+    const DivK divk(k > 0 ? k : 1);
     T *area = areas + (mine ? ring_warp_offset<Gm>(grid, (int)blockIdx.x, lane, ntiles) : 0);
     int fnext = 0, snext = 0;                             // next feed chunk to stage / next output chunk to publish (local time of its first iteration)
     unsigned seen = 0;                                    // last value read from the left band's counter
@@ -178,7 +182,7 @@ __device__ __forceinline__ void ring_comm_warp(typename P::real *u, typename P::
             if (snext + n_pub * CH > lt_end) n_pub = (lt_end - snext) / CH;
             if (fnext < lt_end && fnext + CH - CAP <= k0) {             // the ring slots of the chunk are consumed
                 const int s = fnext / NJI;
-                f_p = s / k;
+                f_p = divk(s);
                 f_band = first + (s - f_p * k) * stride;
                 if (f_p == 0) f_ready = true;                           // the upright triangle takes no row inputs
                 else {
@@ -202,7 +206,7 @@ __device__ __forceinline__ void ring_comm_warp(typename P::real *u, typename P::
         // ---- publish: the computing warp stored its chunk(s) before it released K0 and this lane acquired K0, so the release below
         // orders those stores before the counter for every observer (causality is cumulative across the two scopes)
         for (; n_pub > 0; --n_pub, snext += CH) {
-            const int s = snext / NJI, p = s / k;
+            const int s = snext / NJI, p = divk(s);
             if (p < nph - 1) st_release_gpu(prog + first + (s - p * k) * stride, (unsigned)(p * NCH + (snext & (NJI - 1)) / CH + 1));
         }
         // ---- stage the feeds whose chunk the left band has published (the acquire loads above order the copies behind it for the
@@ -296,10 +300,11 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
         __syncwarp();
     }
 
+    const DivK divk(k);
     int p_cur = 0, lo = L, hi = 0x3fffffff;               // this lane's tile: phase, and the tiers (lo, hi] it updates
     bool interior = false;                               // p_cur is a diamond phase: every point of the tile is updated
     auto set_phase = [&](int s) {
-        p_cur = s / k;
+        p_cur = divk(s);
         lo = p_cur == 0 ? L : 0;
         hi = p_cur < q ? 0x3fffffff : (p_cur == q ? L + rt : rt);
         interior = p_cur > 0 && p_cur < q;
@@ -346,7 +351,7 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
         {
             const int lt0 = K0 - CH * (1 + Gm::LAGC);
             if (lt0 >= 0 && lt0 < lt_end) {
-                const int s = lt0 / NJI, p = s / k;
+                const int s = lt0 / NJI, p = divk(s);
                 if (p < nph - 1) {
                     const int64_t g0 = g0_of(first + (s - p * k) * stride, p);
                     const int it0 = lt0 & (NJI - 1);
@@ -374,9 +379,11 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
             const int need_feed = K0 < lt_end ? (K0 + CH < lt_end ? K0 + CH : lt_end) : 0;
             SpinWatch polls;
             bool dead = false;
+#ifndef RING_EXP_NOWAIT                                   // (experiment: the rate with a free exchange -- results are wrong)
             while ((int)ld_acquire_cta_shared(&my->feed) < need_feed) {
                 if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
             }
+#endif
             if (__any_sync(0xffffffffu, dead)) return;
         }
 
@@ -385,10 +392,11 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
         bool steady = K0 >= 31 && K0 + CH - 1 < lt_end;
         const bool swapchunk = k > 1 && (K0 & (NJI - 1)) < 32;
         if (steady) {
-            const int pa = ((K0 - 31) / NJI) / k, pb = ((K0 + CH - 1) / NJI) / k;
+            const int pa = divk((K0 - 31) / NJI), pb = divk((K0 + CH - 1) / NJI);
             steady = pa > 0 && pb < q;
         }
         if (steady) {
+            constexpr bool ONE_LOOP = P::GROUPED;
             auto steady_chunk = [&](auto swap_tag) {
                 constexpr bool SWAP = decltype(swap_tag)::value;
                 int J = (K0 - lane) & (NJI - 1);
@@ -407,7 +415,7 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
                                 const T r = shfl_up1(keep[sr][kk][rho]);
                                 recv[sr][kk][rho] = lane == 0 ? f : r;
                             }
-                    if (SWAP && J == 0) swap_bands((K0 + it - lane) / NJI);
+                    if (SWAP && (!ONE_LOOP || swapchunk) && J == 0) swap_bands((K0 + it - lane) / NJI);
                     band_super_rows<P, PW, SR, true>(X, recv, keep, c, lane * NP + SR * J + 1, 0, 0);
                     if (lane == 31) {
                         T *op = outr + os * SR * D;
@@ -421,10 +429,12 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
                     J = (J + 1) & (NJI - 1);
                     fs = (fs + 1) & (CAP - 1);
                     os = (os + 1) & (OCAP - 1);
-                    if (SWAP) __syncwarp();               // lane l+1 reads the hand-over slot lane l wrote this iteration
+                    if (SWAP && (!ONE_LOOP || swapchunk)) __syncwarp();   // lane l+1 reads the hand-over slot lane l wrote this iteration
                 }
             };
-            if (swapchunk) steady_chunk(std::true_type{});
+            // Euler's loop body is 40 KB of code: two instances of it, taken in turn by a warp with k > 1 bands, thrash the instruction
+            // cache (ncu, fp64, nx = 2^20: `no_instruction` the top stall, 28 % of the samples) -- one instance, the swap a run-time flag
+            if (ONE_LOOP || swapchunk) steady_chunk(std::true_type{});
             else steady_chunk(std::false_type{});
             continue;
         }
@@ -487,7 +497,7 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
     __syncwarp();
     for (int lt0 = ((lt_end + 31 + CH - 1) / CH) * CH - CH * (1 + Gm::LAGC); lt0 < lt_end; lt0 += CH) {
         if (lt0 < 0) continue;
-        const int s = lt0 / NJI, p = s / k;
+        const int s = lt0 / NJI, p = divk(s);
         if (p >= nph - 1) continue;
         const int64_t g0 = g0_of(first + (s - p * k) * stride, p);
         const int it0 = lt0 & (NJI - 1);

@@ -10,12 +10,16 @@ from gpu_util import TOL, assert_bits_equal, rel_max, to_dev
 pytestmark = pytest.mark.gpu
 
 
-def _run(nx, ny, dtype, nsteps, W=None, fo=0.2, u0=None):
+KERNELS = {"warp": sw.KERNEL2D_WARP, "smem": sw.KERNEL2D_SMEM}     # W = 32 only; narrower tiles always run on the shared-memory kernels
+
+
+def _run(nx, ny, dtype, nsteps, W=None, fo=0.2, u0=None, kernel="warp"):
     import torch
     dx, dt = wl.heat2d_grid(max(nx, ny), fo)
     u0 = wl.heat2d_field(nx, ny).astype(dtype) if u0 is None else u0
     with sw.Solver2D(nx, ny, dx, dt, dtype=sw.F64 if dtype == np.float64 else sw.F32) as s:
         u = to_dev(u0)
+        s.set_option(sw.OPT2D_KERNEL, KERNELS[kernel])
         if W is None:
             s.naive_run(u, nsteps)
         else:
@@ -42,9 +46,15 @@ def test_classic_2d_matches_oracle(nx, ny, nsteps, dtype):
     (128, 64, 32, 16 * 2 + 7),
     (512, 512, 32, 16 * 5 + 3),
     (256, 1024, 16, 8 * 7),
+    (32, 32, 32, 16 * 3),    # one 32 x 32 tile wrapping onto itself: every halo of the register kernel is the tile's own far side
+    (64, 32, 32, 16),        # one half-cycle: pyramid, bridges, inverted pyramid
+    (32, 128, 32, 16 * 4 + 1),
 ])
-def test_swept_2d_equals_classic_and_oracle(nx, ny, W, nsteps, dtype):
-    got, info = _run(nx, ny, dtype, nsteps, W=W)
+@pytest.mark.parametrize("kernel", ["warp", "smem"])
+def test_swept_2d_equals_classic_and_oracle(nx, ny, W, nsteps, dtype, kernel):
+    if kernel == "smem" and W != 32:
+        pytest.skip("W < 32 has one kernel family")
+    got, info = _run(nx, ny, dtype, nsteps, W=W, kernel=kernel)
     ref, _ = _run(nx, ny, dtype, nsteps)
     L = W // 2
     assert info["launches_last_call"] == nsteps % L + 1 + 2 * (nsteps // L)       # remainder + pyramids + (bridges, octahedra) per half-cycle
@@ -63,7 +73,9 @@ def test_swept_2d_full_size_sampled_against_the_oracle():
     u0 = rng.uniform(-1, 1, (n, n))
     got, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0)
     ref, _ = _run(n, n, np.float64, nsteps, u0=u0)
-    assert_bits_equal(got, ref, "swept 2-D vs classic at 4096^2")
+    assert_bits_equal(got, ref, "swept 2-D (register kernel) vs classic at 4096^2")
+    smem, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0, kernel="smem")
+    assert_bits_equal(smem, ref, "swept 2-D (shared-memory kernel) vs classic at 4096^2")
     dx, dt = wl.heat2d_grid(n, 0.2)
     for cy, cx in ((0, 0), (n // 2 + 16, n // 2 + 16)):
         iy, ix = (cy - M // 2 + np.arange(M)) % n, (cx - M // 2 + np.arange(M)) % n
@@ -84,3 +96,24 @@ def test_illegal_arguments_2d():
                 s.swept_run(u, 10, bad)
         with pytest.raises(sw.SweptError):
             s.naive_run(u.float(), 1)
+        with pytest.raises(sw.SweptError):
+            s.set_option(sw.OPT2D_KERNEL, 7)
+
+
+def test_the_two_2d_kernels_agree():
+    """The register kernel and the shared-memory kernel run the same regions in the same tier order with the same store rule:
+    identical fields after 1, 2 and 3 half-cycles (odd and even closing alignment)."""
+    import torch
+    nx = ny = 128
+    dx, dt = wl.heat2d_grid(nx, 0.2)
+    u0 = wl.heat2d_field(nx, ny)
+    for K in (1, 2, 3):
+        outs = []
+        for kern in ("warp", "smem"):
+            with sw.Solver2D(nx, ny, dx, dt) as s:
+                s.set_option(sw.OPT2D_KERNEL, KERNELS[kern])
+                u = to_dev(u0)
+                s.swept_run(u, 16 * K, 32)
+                torch.cuda.synchronize()
+                outs.append(u.cpu().numpy())
+        assert_bits_equal(outs[0], outs[1], f"register vs shared-memory 2-D kernels, {K} half-cycles")
