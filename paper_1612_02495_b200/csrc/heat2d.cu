@@ -34,12 +34,28 @@ namespace {
 
 enum { R_PYRAMID = 0, R_BRIDGES = 1, R_INVERTED = 2, R_OCTAHEDRON = 3 };
 
+// Classic path: a thread updates 16 bytes of consecutive x points (2 doubles / 4 floats): one aligned vector load each for its own
+// row and the rows above and below, two scalar loads for the E / W ends (L1 hits), one vector store -- the 1-D classic kernel's
+// layout (naive.cu).  With one point per thread the kernel was bound by instruction issue (fp64 0.60, fp32 0.34 of the HBM figure).
+template <class T> struct Vec16;
+template <> struct Vec16<double> { using type = double2; static constexpr int N = 2; };
+template <> struct Vec16<float> { using type = float4; static constexpr int N = 4; };
+
 template <class T>
 __global__ void __launch_bounds__(256) classic2d_kernel(const T *__restrict__ src, T *__restrict__ dst, int64_t nx, int64_t ny, typename Heat2D<T>::Consts c) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, j = (int64_t)blockIdx.y * blockDim.y + threadIdx.y;
-    if (i >= nx || j >= ny) return;
-    const int64_t ie = (i + 1) & (nx - 1), iw = (i - 1) & (nx - 1), jn = (j + 1) & (ny - 1), js = (j - 1) & (ny - 1);
-    dst[j * nx + i] = Heat2D<T>::point(c, src[j * nx + i], src[j * nx + ie], src[j * nx + iw], src[jn * nx + i], src[js * nx + i]);
+    using V = typename Vec16<T>::type;
+    constexpr int N = Vec16<T>::N;
+    const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * N, j = (int64_t)blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= nx || j >= ny) return;                       // nx is a power of two >= 8: a multiple of N
+    const int64_t jn = (j + 1) & (ny - 1), js = (j - 1) & (ny - 1);
+    const V vc = *reinterpret_cast<const V *>(src + j * nx + i), vn = *reinterpret_cast<const V *>(src + jn * nx + i), vs = *reinterpret_cast<const V *>(src + js * nx + i);
+    const T *pc = reinterpret_cast<const T *>(&vc), *pn = reinterpret_cast<const T *>(&vn), *ps = reinterpret_cast<const T *>(&vs);
+    const T uw = src[j * nx + ((i - 1) & (nx - 1))], ue = src[j * nx + ((i + N) & (nx - 1))];
+    V out;
+    T *po = reinterpret_cast<T *>(&out);
+#pragma unroll
+    for (int k = 0; k < N; ++k) po[k] = Heat2D<T>::point(c, pc[k], k < N - 1 ? pc[k < N - 1 ? k + 1 : k] : ue, k > 0 ? pc[k > 0 ? k - 1 : k] : uw, pn[k], ps[k]);
+    *reinterpret_cast<V *>(dst + j * nx + i) = out;
 }
 
 // One region kind on the tiles whose origin is (ox, oy) + (tile index) * W.  REGION = R_BRIDGES: blockIdx.z = 0 runs the x-bridges
@@ -116,14 +132,16 @@ __device__ __forceinline__ void tier32(T (&a0)[32], T (&a1)[32], const int lane,
                                        const T *hl, const T *hr, const typename Heat2D<T>::Consts &c) {
     T(&src)[32] = SRC0 ? a0 : a1;
     T(&dst)[32] = SRC0 ? a1 : a0;
-    const bool act = lane >= xa && lane < xb;
+    // bit y of `rows`: row y is in [ya, yb) (warp-uniform); `mine`: ... and this lane is in [xa, xb)
+    const unsigned rows = (yb >= 32 ? 0xffffffffu : (1u << yb) - 1u) & ~((1u << ya) - 1u);
+    const unsigned mine = (lane >= xa && lane < xb) ? rows : 0u;
     // Rows in groups of RG: one warp-uniform branch per group, so that the group's 2 RG shuffles and RG dependent chains
     // (shuffle -> 2 adds -> add -> fma) overlap -- with a branch per row every chain ran exposed (ncu: `wait` 3.3 per issue, FP64 pipe
     // 10 %); rows of a group outside [ya, yb) are computed and dropped (3 rows per tier on average).
-    constexpr int RG = 4;
+    constexpr int RG = sizeof(T) == 4 ? 8 : 4;
 #pragma unroll
     for (int g = 0; g < 32 / RG; ++g) {
-        if (RG * g + RG > ya && RG * g < yb) {            // warp-uniform
+        if ((rows >> (RG * g)) & ((1u << RG) - 1u)) {     // warp-uniform
             T e[RG], w[RG], v[RG];
 #pragma unroll
             for (int r = 0; r < RG; ++r) {
@@ -144,7 +162,7 @@ __device__ __forceinline__ void tier32(T (&a0)[32], T (&a1)[32], const int lane,
 #pragma unroll
             for (int r = 0; r < RG; ++r) {
                 const int y = RG * g + r;
-                if (act && y >= ya && y < yb) dst[y] = v[r];
+                if ((mine >> y) & 1u) dst[y] = v[r];   // (a predicate on the fma itself -- inline PTX -- is turned back into these selects by ptxas)
             }
         }
     }
@@ -152,17 +170,11 @@ __device__ __forceinline__ void tier32(T (&a0)[32], T (&a1)[32], const int lane,
 
 // Tiles of origin (ox, oy) + (tile index) * 32; REGION = R_BRIDGES: tiles [0, ntiles) are the x-bridges at origin (ox, oy), tiles
 // [ntiles, 2 ntiles) the y-bridges at origin (oy, ox).
-template <class T, int REGION>
-__global__ void __launch_bounds__(32 * WARPS2D) swept2d_warp_kernel(T *__restrict__ p0, T *__restrict__ p1, int64_t nx, int64_t ny, int ox, int oy, int tiles_x, int64_t ntiles,
-                                                                     typename Heat2D<T>::Consts c) {
+template <class T, int REGION, bool ybridge>
+__device__ __forceinline__ void tile32(T *__restrict__ p0, T *__restrict__ p1, const int64_t nx, const int64_t ny, const int ox, const int oy, const int tiles_x, const int64_t t,
+                                       T (*halo)[32], const int lane, const typename Heat2D<T>::Consts &c) {
     constexpr int W = 32, L = 16, C = 16;
     constexpr bool HALO_REGION = REGION == R_INVERTED || REGION == R_OCTAHEDRON;
-    __shared__ T halo[WARPS2D][2][32];
-    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
-    int64_t t = (int64_t)blockIdx.x * WARPS2D + warp;
-    if (t >= ntiles * (REGION == R_BRIDGES ? 2 : 1)) return;
-    const bool ybridge = REGION == R_BRIDGES && t >= ntiles;
-    if (ybridge) t -= ntiles;
     const int64_t gx0 = (t % tiles_x) * W + (ybridge ? oy : ox), gy0 = (t / tiles_x) * W + (ybridge ? ox : oy);
     const int64_t mx = nx - 1, my = ny - 1;
     auto gidx = [&](int lx, int ly) -> int64_t { return ((gy0 + ly) & my) * nx + ((gx0 + lx) & mx); };
@@ -174,12 +186,12 @@ __global__ void __launch_bounds__(32 * WARPS2D) swept2d_warp_kernel(T *__restric
         a1[y] = REGION != R_PYRAMID ? p1[g] : T(0);
     }
     T hS = T(0), hN = T(0);
-    const T *hl = halo[warp][0], *hr = halo[warp][1];
+    const T *hl = halo[0], *hr = halo[1];
     if (HALO_REGION) {                                    // tier L reads plane (L - 1) & 1 = 1 one point beyond the tile
         hS = p1[gidx(lane, -1)];
         hN = p1[gidx(lane, W)];
-        halo[warp][0][lane] = p1[gidx(-1, lane)];
-        halo[warp][1][lane] = p1[gidx(W, lane)];
+        halo[0][lane] = p1[gidx(-1, lane)];
+        halo[1][lane] = p1[gidx(W, lane)];
         __syncwarp();
     }
     constexpr int S1 = REGION == R_OCTAHEDRON ? 2 * L - 1 : (REGION == R_INVERTED ? L : L - 1);   // (a bridge's tier L is empty)
@@ -224,11 +236,25 @@ __global__ void __launch_bounds__(32 * WARPS2D) swept2d_warp_kernel(T *__restric
     }
 }
 
+template <class T, int REGION>
+__global__ void __launch_bounds__(32 * WARPS2D, sizeof(T) == 4 ? 2 : 1) swept2d_warp_kernel(T *__restrict__ p0, T *__restrict__ p1, int64_t nx, int64_t ny, int ox, int oy, int tiles_x, int64_t ntiles,
+                                                                     typename Heat2D<T>::Consts c) {
+    __shared__ T halo[WARPS2D][2][32];
+    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
+    const int64_t t = (int64_t)blockIdx.x * WARPS2D + warp;
+    if (t >= ntiles * (REGION == R_BRIDGES ? 2 : 1)) return;
+    // the two kinds of bridge are two instances of the tile code: with the kind a run-time value the compiler re-derived it (and
+    // the rectangle) from the block and thread index inside every row group rather than spend registers on it
+    if (REGION == R_BRIDGES && t >= ntiles) tile32<T, REGION, true>(p0, p1, nx, ny, ox, oy, tiles_x, t - ntiles, halo[warp], lane, c);
+    else tile32<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, halo[warp], lane, c);
+}
+
 template <class T> typename Heat2D<T>::Consts consts_of(const swept2d_ctx *h) { return *reinterpret_cast<const typename Heat2D<T>::Consts *>(h->cb.bytes); }
 
 template <class T> cudaError_t classic2d(swept2d_ctx *h, void *d_u, int64_t nsteps, cudaStream_t st, int64_t *launches) {
     T *a = (T *)d_u, *b = (T *)h->work;
-    const dim3 block(32, 8), grid((unsigned)((h->nx + 31) / 32), (unsigned)((h->ny + 7) / 8));
+    constexpr int N = Vec16<T>::N;
+    const dim3 block(32, 8), grid((unsigned)((h->nx / N + 31) / 32), (unsigned)((h->ny + 7) / 8));
     for (int64_t m = 0; m < nsteps; ++m) {
         classic2d_kernel<T><<<grid, block, 0, st>>>(a, b, h->nx, h->ny, consts_of<T>(h));
         T *t = a; a = b; b = t;
