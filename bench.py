@@ -96,6 +96,8 @@ def parse():
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="SWEPT_OPT_BLOCKS_PER_SM for the per-tile kernels (0 = none / tuned)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
+    ap.add_argument("--probe", action="store_true", help="print the library's microbenchmarks as one JSON line: FP64 / FP32 FMA-chain peaks, shared-memory read peak, "
+                    "latency probes (swept_measure_latencies): the denominators and bounds DESIGN.md quotes")
     ap.add_argument("--heat2d", action="store_true", help="secondary measurement (SURVEY.md section 8(f) NEXT-4): the 2-D swept rule against the classic "
                     "2-D kernel on an nx x nx periodic grid (--nx, default 8192; --nsteps, default 800), one JSON line")
     return ap.parse_args()
@@ -325,6 +327,14 @@ def run_sweep(args):
     out = {"problem": args.problem, "dtype": args.dtype, "unit": "GPts*steps/s", "rows": rows}
     with open(os.path.join(ROOT, "gpurun_out", f"sweep_{args.problem}_{args.dtype}.json"), "w") as f:
         json.dump(out, f, indent=1)
+    with open(os.path.join(ROOT, "gpurun_out", f"sweep_{args.problem}_{args.dtype}.csv"), "w") as f:      # the table profiles/sweeps/ keeps
+        f.write("problem,dtype,log2_nx,nsteps,path,tile_width,launch,GPts_steps_per_s\n")
+        for r in rows:
+            f.write(f"{args.problem},{args.dtype},{r['log2_nx']},{r['nsteps']},classic,,plain,{r['naive']:.4f}\n")
+            f.write(f"{args.problem},{args.dtype},{r['log2_nx']},{r['nsteps']},classic,,graph,{r['naive_graph']:.4f}\n")
+            for k, v in r["swept"].items():
+                kname, W, launch = k.split("/")
+                f.write(f"{args.problem},{args.dtype},{r['log2_nx']},{r['nsteps']},{kname},{W[2:]},{launch},{v:.4f}\n")
     print(f"| nx | classic (plain launches) | classic (graph) | paper-style swept (smem, plain) | best swept | config | speedup vs classic | vs classic graph |")
     print("|---|---:|---:|---:|---:|---|---:|---:|")
     for r in rows:
@@ -398,6 +408,13 @@ def run_stress(args):
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     with open(os.path.join(ROOT, "gpurun_out", "stress.json"), "w") as f:
         json.dump({"unit": "GPts*steps/s", "rows": rows}, f, indent=1)
+    with open(os.path.join(ROOT, "gpurun_out", "stress_config5.csv"), "w") as f:
+        f.write("problem,dtype,nx,nsteps,path,tile_width,blocks_per_sm_cap,GPts_steps_per_s\n")
+        for r in rows:
+            f.write(f"{r['problem']},{r['dtype']},{r['nx']},{r['nsteps']},classic(graph),,,{r['classic_graph']:.4f}\n")
+            for k, v in r["results"].items():
+                kname, W, cap = k.split("/")
+                f.write(f"{r['problem']},{r['dtype']},{r['nx']},{r['nsteps']},{kname},{W[2:]},{cap[4:]},{v:.4f}\n")
     print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: ring | band | chain (W, cap) | smem (W, cap) |")
     print("|---|---|---:|---:|---|---:|---|---|---|---|")
     for r in rows:
@@ -465,6 +482,15 @@ def run_heat2d(args):
 
 def main():
     args = parse()
+    if args.probe:
+        import torch
+        import paper_1612_02495_b200 as sw
+        torch.cuda.set_device(0)
+        print(json.dumps({"alu_peak_f64_Tinstr_s": sw.measure_alu_peak(sw.F64)["instr_per_s"] / 1e12, "alu_peak_f32_Tinstr_s": sw.measure_alu_peak(sw.F32)["instr_per_s"] / 1e12,
+                          "nominal_f64_Tinstr_s": 148 * 64 * 1.965e-3, "nominal_f32_Tinstr_s": 148 * 128 * 1.965e-3,
+                          "smem_peak_GBps": sw.measure_smem_peak()["bytes_per_s"] / 1e9, "smem_nominal_GBps": 148 * 128 * 1.965,
+                          "latency_cycles": sw.measure_latencies()}))
+        return
     if args.heat2d:
         run_heat2d(args)
         return

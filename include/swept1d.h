@@ -238,6 +238,12 @@ int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms, void *cud
  * in *ms (may be NULL).  SYNCHRONISES. */
 int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cuda_stream);
 
+/* Latency probes, in SM clock cycles per operation, one warp alone on its SM (cycles[0..4], a host array of 5 doubles):
+ * [0] a dependent DFMA; [1] the heat update's chain DADD -> DFMA; [2] a dependent 64-bit warp shuffle; [3] a lock-step tier
+ * (two 64-bit shuffles -> DADD -> DFMA); [4] a tier exchanged through shared memory with one block barrier, 256 threads.
+ * They bound what any decomposition of a small grid can reach.  SYNCHRONISES. */
+int swept_measure_latencies(double *cycles, void *cuda_stream);
+
 /* Free the workspace and the handle.  The caller must have synchronised every stream it used. */
 int swept_destroy(swept_handle_t h);
 

@@ -32,7 +32,7 @@ PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}
 SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
-    "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak",
+    "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak", "swept_measure_latencies",
     # include/swept2d.h
     "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy",
 )
@@ -114,6 +114,7 @@ def lib() -> ctypes.CDLL:
     L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     L.swept_problem_info.argtypes = [ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
     L.swept_measure_smem_peak.argtypes = [ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
+    L.swept_measure_latencies.argtypes = [ctypes.POINTER(dbl), vp]
     L.swept2d_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, ctypes.POINTER(_Params2D)]
     L.swept2d_run.argtypes = [vp, vp, i64, ci, vp]
     L.naive2d_run.argtypes = [vp, vp, i64, vp]
@@ -307,6 +308,14 @@ def measure_smem_peak(stream=None) -> dict:
     bps, ms = ctypes.c_double(0), ctypes.c_double(0)
     _check(lib().swept_measure_smem_peak(ctypes.byref(bps), ctypes.byref(ms), _stream_ptr(stream)))
     return {"bytes_per_s": bps.value, "ms": ms.value}
+
+
+def measure_latencies(stream=None) -> dict:
+    """Latency probes (SM cycles per dependent operation, one warp): see swept_measure_latencies in include/swept1d.h."""
+    c = (ctypes.c_double * 5)()
+    _check(lib().swept_measure_latencies(c, _stream_ptr(stream)))
+    names = ("dfma", "dadd_dfma", "shfl64", "lockstep_tier_2shfl_dadd_dfma", "smem_tier_1barrier_256thr")
+    return dict(zip(names, (float(v) for v in c)))
 
 
 def plan(problem: int, nx: int, nsteps: int, tile_width: int, *, dtype: int = F64, kernel: int = KERNEL_WAVE, chain: int = CHAIN_RING) -> list:

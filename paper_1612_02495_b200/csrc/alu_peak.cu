@@ -102,6 +102,55 @@ cudaError_t run_smem_peak(int sm_count, double *bytes_per_s, double *ms_out, cud
     return cudaSuccess;
 }
 
+// Latency probes (one warp, dependent chains, clock64 around N repetitions): the numbers behind DESIGN.md's small-grid bound.
+//   [0] dependent DFMA                      [1] the heat update's chain: DADD -> DFMA (+ an independent DMUL)
+//   [2] dependent 64-bit __shfl_up          [3] a lock-step tier: two 64-bit shuffles -> DADD -> DFMA
+//   [4] a tier through shared memory with one block barrier, 256 threads (store, barrier, two loads, DADD, DFMA)
+template <int WHICH>
+__global__ void latency_probe_kernel(double *out, double a, double b, int n) {
+    __shared__ double sh[2][1024 + 2];
+    double x = (double)threadIdx.x, l = 1.0, r = 2.0;
+    const long long t0 = clock64();
+    for (int i = 0; i < n; ++i) {
+        if (WHICH == 0) x = fma(x, a, b);
+        else if (WHICH == 1) { const double t = x + l, v = b * r; x = fma(a, t, v); }
+        else if (WHICH == 2) x = __shfl_up_sync(0xffffffffu, x, 1);
+        else if (WHICH == 3) {
+            const double lo = __shfl_up_sync(0xffffffffu, x, 1), hi = __shfl_down_sync(0xffffffffu, x, 1);
+            const double t = lo + hi, v = b * x;
+            x = fma(a, t, v);
+        } else {
+            double *s = sh[i & 1];
+            s[threadIdx.x + 1] = x;
+            __syncthreads();
+            const double t = s[threadIdx.x] + s[threadIdx.x + 2], v = b * x;
+            x = fma(a, t, v);
+        }
+    }
+    const long long t1 = clock64();
+    if (threadIdx.x == 0) out[WHICH] = (double)(t1 - t0) / n;
+    if (x == 123456789.0) out[7] = x;
+}
+
+cudaError_t run_latency_probes(double *cycles, cudaStream_t st) {
+    double *d = nullptr;
+    cudaError_t e = cudaMalloc(&d, 8 * sizeof(double));
+    if (e != cudaSuccess) return e;
+    cudaMemsetAsync(d, 0, 8 * sizeof(double), st);
+    constexpr int N = 4096;
+    for (int rep = 0; rep < 2; ++rep) {                       // the first pass warms the instruction cache
+        latency_probe_kernel<0><<<1, 32, 0, st>>>(d, 1.0000001, 1e-9, N);
+        latency_probe_kernel<1><<<1, 32, 0, st>>>(d, 0.25, 0.5, N);
+        latency_probe_kernel<2><<<1, 32, 0, st>>>(d, 0.0, 0.0, N);
+        latency_probe_kernel<3><<<1, 32, 0, st>>>(d, 0.25, 0.5, N);
+        latency_probe_kernel<4><<<1, 256, 0, st>>>(d, 0.25, 0.5, N);
+    }
+    e = cudaMemcpyAsync(cycles, d, 5 * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d);
+    return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st) {
     return dtype == SWEPT_F64 ? run_peak<double>(sm_count, instr_per_s, ms, st) : run_peak<float>(sm_count, instr_per_s, ms, st);
 }

@@ -731,6 +731,13 @@ extern "C" int swept_measure_alu_peak(int dtype, double *instr_per_s, double *ms
     return SWEPT_OK;
 }
 
+extern "C" int swept_measure_latencies(double *cycles, void *cuda_stream) {
+    if (!cycles) return fail(SWEPT_EINVAL, "swept_measure_latencies: cycles is NULL");
+    const cudaError_t e = run_latency_probes(cycles, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_measure_latencies");
+    return SWEPT_OK;
+}
+
 extern "C" int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cuda_stream) {
     int dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);

@@ -97,6 +97,7 @@ int swept_fail(int code, const char *fmt, ...) __attribute__((format(printf, 2, 
 // FMA-chain microbenchmark (alu_peak.cu)
 cudaError_t run_alu_peak(int dtype, int sm_count, double *instr_per_s, double *ms, cudaStream_t st);
 cudaError_t run_smem_peak(int sm_count, double *bytes_per_s, double *ms, cudaStream_t st);
+cudaError_t run_latency_probes(double *cycles, cudaStream_t st);
 
 inline int radius_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }
 inline int stages_of(int problem) { return problem == SWEPT_HEAT ? 1 : 2; }
