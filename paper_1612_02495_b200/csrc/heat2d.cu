@@ -13,7 +13,6 @@
 #include <string.h>
 
 #include <new>
-#include <type_traits>
 
 #include "../../include/swept2d.h"
 #include "internal.h"
@@ -250,132 +249,6 @@ __global__ void __launch_bounds__(32 * WARPS2D, sizeof(T) == 4 ? 2 : 1) swept2d_
     else tile32<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, halo[warp], lane, c);
 }
 
-// ---- the same tile with plane 1 in shared memory (fp64) --------------------------------------------------------------
-// Two planes of 32 doubles are 128 registers per lane: 8 warps per SM, too few to cover the update's dependent chain (ncu: issue slots
-// 45 % used, FP64 pipe 18-24 %).  Here plane 0 (even tiers) stays in registers and plane 1 (odd tiers) lives in a 34 x 34 array of
-// shared memory per warp, halo ring included:
-//   odd tier  (plane 0 -> plane 1): E/W by shuffle, N/S registers, the result stored to shared memory under the lane's row mask
-//                                   (a predicated store: no select);
-//   even tier (plane 1 -> plane 0): the five values are shared-memory loads (own row and the two neighbours' columns; the rows of a
-//                                   group share their N/S loads), the result selected into the register.
-// Half the registers, twice the warps, no shuffles on even tiers, and the halo of tier L (an even tier: it reads plane 1) is just the
-// ring of the shared-memory array.  Only __syncwarp() between tiers.
-constexpr int WARPS2H = 4, PS2H = 34;
-
-template <class T, int REGION, bool ybridge>
-__device__ __forceinline__ void tile32h(T *__restrict__ p0, T *__restrict__ p1, const int64_t nx, const int64_t ny, const int ox, const int oy, const int tiles_x, const int64_t t,
-                                        T *__restrict__ s1, const int lane, const typename Heat2D<T>::Consts &c) {
-    constexpr int W = 32, L = 16, C = 16, PS = PS2H, RG = 4;
-    constexpr bool HALO_REGION = REGION == R_INVERTED || REGION == R_OCTAHEDRON;
-    const int64_t gx0 = (t % tiles_x) * W + (ybridge ? oy : ox), gy0 = (t / tiles_x) * W + (ybridge ? ox : oy);
-    const int64_t mx = nx - 1, my = ny - 1;
-    auto gidx = [&](int lx, int ly) -> int64_t { return ((gy0 + ly) & my) * nx + ((gx0 + lx) & mx); };
-    T *me = s1 + PS + lane + 1;                           // point (lane, y) of plane 1: me[y * PS]
-    T a0[32];
-#pragma unroll
-    for (int y = 0; y < 32; ++y) a0[y] = p0[gidx(lane, y)];
-    if (REGION != R_PYRAMID) {
-#pragma unroll
-        for (int y = 0; y < 32; ++y) me[y * PS] = p1[gidx(lane, y)];
-        if (HALO_REGION) {
-            me[-PS] = p1[gidx(lane, -1)];
-            me[32 * PS] = p1[gidx(lane, W)];
-            s1[(lane + 1) * PS] = p1[gidx(-1, lane)];
-            s1[(lane + 1) * PS + W + 1] = p1[gidx(W, lane)];
-        }
-    }
-    __syncwarp();
-    constexpr int S1 = REGION == R_OCTAHEDRON ? 2 * L - 1 : (REGION == R_INVERTED ? L : L - 1);
-    auto masks = [&](int s, unsigned &rows, unsigned &mine) {
-        int xa, xb, ya, yb;
-        if (REGION == R_PYRAMID) { xa = ya = s; xb = yb = W - s; }
-        else if (REGION == R_BRIDGES) {
-            const int ea = C - s, eb = C + s, sa = s, sb = W - s;
-            xa = ybridge ? sa : ea; xb = ybridge ? sb : eb;
-            ya = ybridge ? ea : sa; yb = ybridge ? eb : sb;
-        } else if (s <= L) { xa = ya = C - s; xb = yb = C + s; }
-        else { xa = ya = s - L; xb = yb = W - (s - L); }
-        rows = (yb >= 32 ? 0xffffffffu : (1u << yb) - 1u) & ~((1u << ya) - 1u);
-        mine = (lane >= xa && lane < xb) ? rows : 0u;
-    };
-#pragma unroll 1
-    for (int s = 1; s <= S1; s += 2) {
-        unsigned rows, mine;
-        masks(s, rows, mine);
-        // ---- odd tier: plane 0 (registers) -> plane 1 (shared memory).  Rows 0 and 31 are never in an odd tier's rectangle.
-#pragma unroll
-        for (int g = 0; g < 32 / RG; ++g) {
-            if ((rows >> (RG * g)) & ((1u << RG) - 1u)) {
-                T e[RG], w[RG];
-#pragma unroll
-                for (int r = 0; r < RG; ++r) {
-                    e[r] = __shfl_down_sync(0xffffffffu, a0[RG * g + r], 1);
-                    w[r] = __shfl_up_sync(0xffffffffu, a0[RG * g + r], 1);
-                }
-#pragma unroll
-                for (int r = 0; r < RG; ++r) {
-                    const int y = RG * g + r;
-                    const T v = Heat2D<T>::point(c, a0[y], e[r], w[r], a0[y < 31 ? y + 1 : 31], a0[y > 0 ? y - 1 : 0]);
-                    if ((mine >> y) & 1u) me[y * PS] = v;
-                }
-            }
-        }
-        __syncwarp();
-        if (s + 1 > S1) break;
-        masks(s + 1, rows, mine);
-        // ---- even tier: plane 1 (shared memory, halo ring included) -> plane 0 (registers)
-#pragma unroll
-        for (int g = 0; g < 32 / RG; ++g) {
-            if ((rows >> (RG * g)) & ((1u << RG) - 1u)) {
-                T cc[RG + 2], e[RG], w[RG];
-#pragma unroll
-                for (int r = 0; r < RG + 2; ++r) cc[r] = me[(RG * g + r - 1) * PS];
-#pragma unroll
-                for (int r = 0; r < RG; ++r) {
-                    e[r] = me[(RG * g + r) * PS + 1];
-                    w[r] = me[(RG * g + r) * PS - 1];
-                }
-#pragma unroll
-                for (int r = 0; r < RG; ++r) {
-                    const int y = RG * g + r;
-                    const T v = Heat2D<T>::point(c, cc[r + 1], e[r], w[r], cc[r + 2], cc[r]);
-                    if ((mine >> y) & 1u) a0[y] = v;
-                }
-            }
-        }
-        __syncwarp();
-    }
-    // ---- store (the rule of tile32)
-    const int x = lane, ux = x < W - 1 - x ? x : W - 1 - x, dx = C - x > x - C + 1 ? C - x : x - C + 1;
-#pragma unroll
-    for (int y = 0; y < 32; ++y) {
-        const int uy = y < W - 1 - y ? y : W - 1 - y, dy = C - y > y - C + 1 ? C - y : y - C + 1;
-        const int umin = ux < uy ? ux : uy, dmax = dx > dy ? dx : dy;
-        int s_lo, s_hi;
-        if (REGION == R_PYRAMID) { s_lo = 1; s_hi = umin; }
-        else if (REGION == R_BRIDGES) { s_lo = ybridge ? dy : dx; s_hi = ybridge ? ux : uy; }
-        else if (REGION == R_INVERTED) { s_lo = dmax; s_hi = L; }
-        else { s_lo = dmax; s_hi = L + umin; }
-        if (s_hi >= s_lo && s_hi >= 1) {
-            const int64_t g = gidx(x, y);
-            const bool odd = (s_hi & 1) != 0;
-            if (odd || s_hi > s_lo) p1[g] = me[y * PS];
-            if (!odd || s_hi > s_lo) p0[g] = a0[y];
-        }
-    }
-}
-
-template <class T, int REGION>
-__global__ void __launch_bounds__(32 * WARPS2H, sizeof(T) == 8 ? 3 : 4) swept2d_hybrid_kernel(T *__restrict__ p0, T *__restrict__ p1, int64_t nx, int64_t ny, int ox, int oy, int tiles_x, int64_t ntiles,
-                                                                          typename Heat2D<T>::Consts c) {
-    __shared__ T plane1[WARPS2H][PS2H * PS2H];
-    const int lane = (int)(threadIdx.x & 31), warp = (int)(threadIdx.x >> 5);
-    const int64_t t = (int64_t)blockIdx.x * WARPS2H + warp;
-    if (t >= ntiles * (REGION == R_BRIDGES ? 2 : 1)) return;
-    if (REGION == R_BRIDGES && t >= ntiles) tile32h<T, REGION, true>(p0, p1, nx, ny, ox, oy, tiles_x, t - ntiles, plane1[warp], lane, c);
-    else tile32h<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, plane1[warp], lane, c);
-}
-
 template <class T> typename Heat2D<T>::Consts consts_of(const swept2d_ctx *h) { return *reinterpret_cast<const typename Heat2D<T>::Consts *>(h->cb.bytes); }
 
 template <class T> cudaError_t classic2d(swept2d_ctx *h, void *d_u, int64_t nsteps, cudaStream_t st, int64_t *launches) {
@@ -409,37 +282,28 @@ template <class T, int W> cudaError_t sweep2d(swept2d_ctx *h, void *d_u, int64_t
     return cudaGetLastError();
 }
 
-template <class T, bool HYBRID> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K, cudaStream_t st, int64_t *launches) {
+template <class T> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K, cudaStream_t st, int64_t *launches) {
     if (K <= 0) return cudaSuccess;
-    constexpr int W = 32, WPB = HYBRID ? WARPS2H : WARPS2D;
+    constexpr int W = 32;
     T *p0 = (T *)d_u, *p1 = (T *)h->work;
     const int tiles_x = (int)(h->nx / W);
     const int64_t ntiles = (h->nx / W) * (h->ny / W);
-    const dim3 block(32 * WPB), grid((unsigned)((ntiles + WPB - 1) / WPB)), grid2((unsigned)((2 * ntiles + WPB - 1) / WPB));
+    const dim3 block(32 * WARPS2D), grid((unsigned)((ntiles + WARPS2D - 1) / WARPS2D)), grid2((unsigned)((2 * ntiles + WARPS2D - 1) / WARPS2D));
     const typename Heat2D<T>::Consts c = consts_of<T>(h);
-    auto launch = [&](auto region, dim3 g, int ox, int oy) {
-        constexpr int R = decltype(region)::value;
-        if constexpr (HYBRID) swept2d_hybrid_kernel<T, R><<<g, block, 0, st>>>(p0, p1, h->nx, h->ny, ox, oy, tiles_x, ntiles, c);
-        else swept2d_warp_kernel<T, R><<<g, block, 0, st>>>(p0, p1, h->nx, h->ny, ox, oy, tiles_x, ntiles, c);
-    };
-    launch(std::integral_constant<int, R_PYRAMID>{}, grid, 0, 0);
+    swept2d_warp_kernel<T, R_PYRAMID><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, 0, 0, tiles_x, ntiles, c);
     ++*launches;
     for (int64_t k = 0; k < K; ++k) {
         const int a = (int)(k & 1) * (W / 2), b = W / 2 - a;      // a: the alignment that shrinks in this half-cycle
-        launch(std::integral_constant<int, R_BRIDGES>{}, grid2, b, a);
-        if (k == K - 1) launch(std::integral_constant<int, R_INVERTED>{}, grid, b, b);
-        else launch(std::integral_constant<int, R_OCTAHEDRON>{}, grid, b, b);
+        swept2d_warp_kernel<T, R_BRIDGES><<<grid2, block, 0, st>>>(p0, p1, h->nx, h->ny, b, a, tiles_x, ntiles, c);
+        if (k == K - 1) swept2d_warp_kernel<T, R_INVERTED><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
+        else swept2d_warp_kernel<T, R_OCTAHEDRON><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
         *launches += 2;
     }
     return cudaGetLastError();
 }
 
 template <class T> cudaError_t sweep2d_w(swept2d_ctx *h, void *d_u, int W, int64_t K, cudaStream_t st, int64_t *launches) {
-    if (W == 32 && h->kernel != SWEPT2D_KERNEL_SMEM) {
-        // default: fp64 on the hybrid kernel (plane 1 in shared memory), fp32 with both planes in registers
-        const bool hybrid = h->kernel == SWEPT2D_KERNEL_HYBRID || (h->kernel == SWEPT2D_KERNEL_WARP && sizeof(T) == 8);
-        return hybrid ? sweep2d_warp<T, true>(h, d_u, K, st, launches) : sweep2d_warp<T, false>(h, d_u, K, st, launches);
-    }
+    if (W == 32 && h->kernel != SWEPT2D_KERNEL_SMEM) return sweep2d_warp<T>(h, d_u, K, st, launches);
     switch (W) {
         case 8: return sweep2d<T, 8>(h, d_u, K, st, launches);
         case 16: return sweep2d<T, 16>(h, d_u, K, st, launches);
@@ -526,7 +390,7 @@ extern "C" int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int ti
 
 extern "C" int swept2d_set_option(swept2d_handle_t h, int option, int value) {
     if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_set_option: NULL handle");
-    if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM && value != SWEPT2D_KERNEL_HYBRID && value != SWEPT2D_KERNEL_REGS))
+    if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM))
         return swept_fail(SWEPT_EINVAL, "swept2d_set_option: unknown option %d or value %d", option, value);
     h->kernel = value;
     return SWEPT_OK;

@@ -10,8 +10,7 @@ from gpu_util import TOL, assert_bits_equal, rel_max, to_dev
 pytestmark = pytest.mark.gpu
 
 
-# W = 32 only (narrower tiles always run on the shared-memory kernels); "warp" = the default: hybrid for fp64, regs for fp32
-KERNELS = {"warp": sw.KERNEL2D_WARP, "smem": sw.KERNEL2D_SMEM, "hybrid": sw.KERNEL2D_HYBRID, "regs": sw.KERNEL2D_REGS}
+KERNELS = {"warp": sw.KERNEL2D_WARP, "smem": sw.KERNEL2D_SMEM}     # W = 32 only; narrower tiles always run on the shared-memory kernels
 
 
 def _run(nx, ny, dtype, nsteps, W=None, fo=0.2, u0=None, kernel="warp"):
@@ -51,9 +50,9 @@ def test_classic_2d_matches_oracle(nx, ny, nsteps, dtype):
     (64, 32, 32, 16),        # one half-cycle: pyramid, bridges, inverted pyramid
     (32, 128, 32, 16 * 4 + 1),
 ])
-@pytest.mark.parametrize("kernel", ["hybrid", "regs", "smem"])
+@pytest.mark.parametrize("kernel", ["warp", "smem"])
 def test_swept_2d_equals_classic_and_oracle(nx, ny, W, nsteps, dtype, kernel):
-    if kernel != "smem" and W != 32:
+    if kernel == "smem" and W != 32:
         pytest.skip("W < 32 has one kernel family")
     got, info = _run(nx, ny, dtype, nsteps, W=W, kernel=kernel)
     ref, _ = _run(nx, ny, dtype, nsteps)
@@ -74,10 +73,9 @@ def test_swept_2d_full_size_sampled_against_the_oracle():
     u0 = rng.uniform(-1, 1, (n, n))
     got, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0)
     ref, _ = _run(n, n, np.float64, nsteps, u0=u0)
-    assert_bits_equal(got, ref, "swept 2-D (default: hybrid kernel) vs classic at 4096^2")
-    for kern in ("regs", "smem"):
-        other, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0, kernel=kern)
-        assert_bits_equal(other, ref, f"swept 2-D ({kern} kernel) vs classic at 4096^2")
+    assert_bits_equal(got, ref, "swept 2-D (register kernel) vs classic at 4096^2")
+    smem, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0, kernel="smem")
+    assert_bits_equal(smem, ref, "swept 2-D (shared-memory kernel) vs classic at 4096^2")
     dx, dt = wl.heat2d_grid(n, 0.2)
     for cy, cx in ((0, 0), (n // 2 + 16, n // 2 + 16)):
         iy, ix = (cy - M // 2 + np.arange(M)) % n, (cx - M // 2 + np.arange(M)) % n
@@ -102,8 +100,8 @@ def test_illegal_arguments_2d():
             s.set_option(sw.OPT2D_KERNEL, 7)
 
 
-def test_the_2d_kernel_families_agree():
-    """The warp-per-tile kernels (hybrid, registers) and the shared-memory kernel run the same regions in the same tier order with the same store rule:
+def test_the_two_2d_kernels_agree():
+    """The register kernel and the shared-memory kernel run the same regions in the same tier order with the same store rule:
     identical fields after 1, 2 and 3 half-cycles (odd and even closing alignment)."""
     import torch
     nx = ny = 128
@@ -111,12 +109,11 @@ def test_the_2d_kernel_families_agree():
     u0 = wl.heat2d_field(nx, ny)
     for K in (1, 2, 3):
         outs = []
-        for kern in ("hybrid", "regs", "smem"):
+        for kern in ("warp", "smem"):
             with sw.Solver2D(nx, ny, dx, dt) as s:
                 s.set_option(sw.OPT2D_KERNEL, KERNELS[kern])
                 u = to_dev(u0)
                 s.swept_run(u, 16 * K, 32)
                 torch.cuda.synchronize()
                 outs.append(u.cpu().numpy())
-        assert_bits_equal(outs[0], outs[1], f"hybrid vs register 2-D kernels, {K} half-cycles")
-        assert_bits_equal(outs[0], outs[2], f"hybrid vs shared-memory 2-D kernels, {K} half-cycles")
+        assert_bits_equal(outs[0], outs[1], f"register vs shared-memory 2-D kernels, {K} half-cycles")
