@@ -434,6 +434,8 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
             };
             // Euler's loop body is 40 KB of code: two instances of it, taken in turn by a warp with k > 1 bands, thrash the instruction
             // cache (ncu, fp64, nx = 2^20: `no_instruction` the top stall, 28 % of the samples) -- one instance, the swap a run-time flag
+            // (also for a warp with one band, which never swaps: warps with one and with two bands share an SM, and the plain instance
+            // beside the merged one is the same 84 KB again -- measured: ring 2^19 36.4 -> 26.6)
             if (ONE_LOOP || swapchunk) steady_chunk(std::true_type{});
             else steady_chunk(std::false_type{});
             continue;
