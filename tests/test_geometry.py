@@ -452,3 +452,19 @@ def test_band_schedule_with_one_chunk_per_tile_is_a_cycle_of_waits():
     reason those widths run on the tile-flag kernel (band_grid refuses NCH < 2)."""
     done, _ = _simulate_band_schedule(64, 148, 1, q=3, NJI=32)
     assert not done
+
+
+def test_multiply_high_division_by_the_band_count_is_exact():
+    """DivK (csrc/swept_band.cuh): floor(s / k) = (s * ceil(2^32 / k)) >> 32 for every s with s k < 2^32 -- the range the kernels
+    use it in (s = local tile number < 2^30 / NJI, k = bands per warp).  Checked exhaustively for small s, at the range's edges
+    and on a seeded sample, for every k the band layouts can produce."""
+    rng = np.random.default_rng(1612)
+    for k in list(range(2, 130)) + [255, 256, 1000, 4095, 4096, 65535]:
+        m = ((1 << 32) + k - 1) // k
+        assert m < (1 << 32)
+        top = ((1 << 32) - 1) // k                      # largest s with s k < 2^32
+        samples = np.concatenate([np.arange(0, min(top, 5000)), top - np.arange(0, min(top, 5000)), rng.integers(0, top + 1, 20000),
+                                  (np.arange(1, min(top // k, 3000) + 1) * k - 1), (np.arange(1, min(top // k, 3000) + 1) * k)])
+        samples = samples[(samples >= 0) & (samples <= top)].astype(object)
+        for s in samples[:: max(1, len(samples) // 4000)]:
+            assert (int(s) * m) >> 32 == int(s) // k, (k, s)

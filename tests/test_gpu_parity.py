@@ -226,6 +226,17 @@ def test_alu_peak_microbenchmark_is_plausible():
     assert 1e12 < p64 < 1e14 and 1e12 < p32 < 2e14
 
 
+def test_smem_peak_and_latency_probes_are_plausible():
+    """swept_measure_smem_peak / swept_measure_latencies (include/swept1d.h): the denominators and bounds DESIGN.md quotes."""
+    bw = sw.measure_smem_peak()["bytes_per_s"]
+    assert 5e12 < bw < 1e14
+    lat = sw.measure_latencies()
+    assert set(lat) == {"dfma", "dadd_dfma", "shfl64", "lockstep_tier_2shfl_dadd_dfma", "smem_tier_1barrier_256thr"}
+    assert all(np.isfinite(v) and 1.0 < v < 2000.0 for v in lat.values()), lat
+    assert lat["dfma"] < lat["dadd_dfma"] < lat["lockstep_tier_2shfl_dadd_dfma"], lat       # one op < two dependent ops < shuffle + two ops
+    assert lat["shfl64"] < lat["lockstep_tier_2shfl_dadd_dfma"] < lat["smem_tier_1barrier_256thr"], lat
+
+
 # ------------------------------------------------------------------------------------------------------------
 # launch-free sweep (SWEPT_OPT_CHAIN): flag-ordered persistent kernel
 # ------------------------------------------------------------------------------------------------------------
