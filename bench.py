@@ -456,7 +456,7 @@ def run_heat2d(args):
     with sw.Solver2D(n, n, dx, dt, dtype=sw.F64 if args.dtype == "f64" else sw.F32) as s:
         t = timed(lambda: s.naive_run(u, nsteps))
         res["classic"] = n * n * nsteps / t / 1e9
-        for W, kern, kname in ((32, sw.KERNEL2D_WARP, "register kernel"), (32, sw.KERNEL2D_SMEM, "paper-style smem kernel"), (16, sw.KERNEL2D_SMEM, "paper-style smem kernel"),
+        for W, kern, kname in ((32, sw.KERNEL2D_WARP, "register kernel"), (32, sw.KERNEL2D_COLUMN, "register kernel, one column per lane"), (32, sw.KERNEL2D_SMEM, "paper-style smem kernel"), (16, sw.KERNEL2D_SMEM, "paper-style smem kernel"),
                                (8, sw.KERNEL2D_SMEM, "paper-style smem kernel")):
             s.set_option(sw.OPT2D_KERNEL, kern)
             u.copy_(u0)

@@ -23,7 +23,7 @@ PACK_AUTO, PACK_OFF, PACK_ON = 0, 1, 2
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}
 BC_PERIODIC, BC_INSULATED = 0, 1
-OPT2D_KERNEL, KERNEL2D_WARP, KERNEL2D_SMEM = 0, 0, 1                 # include/swept2d.h: swept2d_set_option
+OPT2D_KERNEL, KERNEL2D_WARP, KERNEL2D_SMEM, KERNEL2D_COLUMN = 0, 0, 1, 2      # include/swept2d.h: swept2d_set_option
 CHAIN_OFF, CHAIN_TILES, CHAIN_BANDS, CHAIN_RING = 0, 1, 2, 3     # values of OPT_CHAIN (include/swept1d.h); CHAIN_RING is the default
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 PROBLEMS = {"heat": HEAT, "ks": KS, "euler": EULER}

@@ -236,7 +236,135 @@ __device__ __forceinline__ void tile32(T *__restrict__ p0, T *__restrict__ p1, c
     }
 }
 
-template <class T, int REGION>
+// ---- the folded tile: two columns per lane, the upper 16 rows folded onto lanes 16..31 ----------------------------------------
+// tile32 above spends 4 shuffles and ~10 bookkeeping instructions per 32-point row on 5 FP instructions.  Here lane (half, l) owns
+// the columns 2l, 2l+1 of the rows r (half 0) or 31 - r (half 1), r = 0..15: a register row r is 64 points.  Of a point pair only
+// the outer E / W neighbours cross lanes (one shuffle each, within the 16-lane half), so shuffles per point halve and the row
+// bookkeeping is shared by two points.  Every rectangle is symmetric about the tile's centre row, so register row r is active in both
+// halves at once ([ya, 32 - ya) = r >= ya) and nothing is wasted by the fold; the upper half runs its rows top-down, which swaps the
+// roles of N and S -- harmless bit for bit, the update adds them (uN + uS = uS + uN).  The seam (rows 15 | 16) is one exchange
+// between the halves per tier and column.
+template <class T> struct alignas(2 * sizeof(T)) Pair2 { T a, b; };
+
+template <class T, bool SRC0, bool HALO>
+__device__ __forceinline__ void tier32f(T (&a0)[16][2], T (&a1)[16][2], const int half, const int l, const int xa, const int xb, const int ya, const T (&hrow)[2],
+                                        const T *hl, const T *hr, const typename Heat2D<T>::Consts &c) {
+    T(&src)[16][2] = SRC0 ? a0 : a1;
+    T(&dst)[16][2] = SRC0 ? a1 : a0;
+    constexpr int RG = sizeof(T) == 4 ? 4 : 2;
+    const unsigned rows = 0xffffu & ~((1u << ya) - 1u);    // register rows ya .. 15 (warp-uniform)
+    const int x0 = 2 * l;
+    const unsigned mine0 = (x0 >= xa && x0 < xb) ? rows : 0u, mine1 = (x0 + 1 >= xa && x0 + 1 < xb) ? rows : 0u;
+    T seam[2];                                            // row 16 for the lower half, row 15 for the upper: the other half's r = 15
+#pragma unroll
+    for (int k = 0; k < 2; ++k) seam[k] = __shfl_xor_sync(0xffffffffu, src[15][k], 16);
+#pragma unroll
+    for (int g = 0; g < 16 / RG; ++g) {
+        if ((rows >> (RG * g)) & ((1u << RG) - 1u)) {     // warp-uniform
+            T eR[RG], wL[RG], v0[RG], v1[RG];
+#pragma unroll
+            for (int q = 0; q < RG; ++q) {
+                const int r = RG * g + q;
+                eR[q] = __shfl_down_sync(0xffffffffu, src[r][0], 1, 16);   // lane l+1's left column: E of my right column
+                wL[q] = __shfl_up_sync(0xffffffffu, src[r][1], 1, 16);     // lane l-1's right column: W of my left column
+                if (HALO) {
+                    const int y = half ? 31 - r : r;
+                    if (l == 0) wL[q] = hl[y];
+                    if (l == 15) eR[q] = hr[y];
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < RG; ++q) {
+                const int r = RG * g + q;
+                const T up0 = r < 15 ? src[r < 15 ? r + 1 : 15][0] : seam[0], up1 = r < 15 ? src[r < 15 ? r + 1 : 15][1] : seam[1];
+                const T dn0 = r > 0 ? src[r > 0 ? r - 1 : 0][0] : hrow[0], dn1 = r > 0 ? src[r > 0 ? r - 1 : 0][1] : hrow[1];
+                v0[q] = Heat2D<T>::point(c, src[r][0], src[r][1], wL[q], up0, dn0);
+                v1[q] = Heat2D<T>::point(c, src[r][1], eR[q], src[r][0], up1, dn1);
+            }
+#pragma unroll
+            for (int q = 0; q < RG; ++q) {
+                const int r = RG * g + q;
+                if ((mine0 >> r) & 1u) dst[r][0] = v0[q];
+                if ((mine1 >> r) & 1u) dst[r][1] = v1[q];
+            }
+        }
+    }
+}
+
+template <class T, int REGION, bool ybridge>
+__device__ __forceinline__ void tile32f(T *__restrict__ p0, T *__restrict__ p1, const int64_t nx, const int64_t ny, const int ox, const int oy, const int tiles_x, const int64_t t,
+                                        T (*halo)[32], const int lane, const typename Heat2D<T>::Consts &c) {
+    constexpr int W = 32, L = 16, C = 16;
+    constexpr bool HALO_REGION = REGION == R_INVERTED || REGION == R_OCTAHEDRON;
+    using V2 = Pair2<T>;
+    const int half = lane >> 4, l = lane & 15, x0 = 2 * l;
+    const int64_t gx0 = (t % tiles_x) * W + (ybridge ? oy : ox), gy0 = (t / tiles_x) * W + (ybridge ? ox : oy);
+    const int64_t mx = nx - 1, my = ny - 1;
+    auto gidx = [&](int lx, int ly) -> int64_t { return ((gy0 + ly) & my) * nx + ((gx0 + lx) & mx); };
+    T a0[16][2], a1[16][2];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int64_t g = gidx(x0, half ? 31 - r : r);    // gx0 and x0 are even: the pair is aligned and does not straddle the wrap
+        const V2 v = *reinterpret_cast<const V2 *>(p0 + g);
+        a0[r][0] = v.a; a0[r][1] = v.b;
+        if (REGION != R_PYRAMID) {
+            const V2 u = *reinterpret_cast<const V2 *>(p1 + g);
+            a1[r][0] = u.a; a1[r][1] = u.b;
+        } else { a1[r][0] = a1[r][1] = T(0); }
+    }
+    T hrow[2] = {T(0), T(0)};                             // row -1 (lower half) / row 32 (upper half) of plane 1, this lane's columns
+    const T *hl = halo[0], *hr = halo[1];
+    if (HALO_REGION) {                                    // tier L reads plane (L - 1) & 1 = 1 one point beyond the tile
+        const V2 u = *reinterpret_cast<const V2 *>(p1 + gidx(x0, half ? W : -1));
+        hrow[0] = u.a; hrow[1] = u.b;
+        halo[0][lane] = p1[gidx(-1, lane)];
+        halo[1][lane] = p1[gidx(W, lane)];
+        __syncwarp();
+    }
+    constexpr int S1 = REGION == R_OCTAHEDRON ? 2 * L - 1 : (REGION == R_INVERTED ? L : L - 1);
+    auto rect = [&](int s, int &xa, int &xb, int &ya) {   // (yb = 32 - ya for every region)
+        if (REGION == R_PYRAMID) { xa = ya = s; xb = W - s; }
+        else if (REGION == R_BRIDGES) {
+            xa = ybridge ? s : C - s; xb = ybridge ? W - s : C + s;
+            ya = ybridge ? C - s : s;
+        } else if (s <= L) { xa = ya = C - s; xb = C + s; }
+        else { xa = ya = s - L; xb = W - (s - L); }
+    };
+#pragma unroll 1
+    for (int s = 1; s <= S1; s += 2) {
+        int xa, xb, ya;
+        rect(s, xa, xb, ya);
+        tier32f<T, true, false>(a0, a1, half, l, xa, xb, ya, hrow, hl, hr, c);
+        if (s + 1 <= S1) {
+            rect(s + 1, xa, xb, ya);
+            if (HALO_REGION && s + 1 == L) tier32f<T, false, true>(a0, a1, half, l, xa, xb, ya, hrow, hl, hr, c);
+            else tier32f<T, false, false>(a0, a1, half, l, xa, xb, ya, hrow, hl, hr, c);
+        }
+    }
+    // ---- store (the rule of tile32): for register row r both halves have uy = r and dy = 16 - r
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int y = half ? 31 - r : r, uy = r, dy = C - r;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const int x = x0 + k, ux = x < W - 1 - x ? x : W - 1 - x, dx = C - x > x - C + 1 ? C - x : x - C + 1;
+            const int umin = ux < uy ? ux : uy, dmax = dx > dy ? dx : dy;
+            int s_lo, s_hi;
+            if (REGION == R_PYRAMID) { s_lo = 1; s_hi = umin; }
+            else if (REGION == R_BRIDGES) { s_lo = ybridge ? dy : dx; s_hi = ybridge ? ux : uy; }
+            else if (REGION == R_INVERTED) { s_lo = dmax; s_hi = L; }
+            else { s_lo = dmax; s_hi = L + umin; }
+            if (s_hi >= s_lo && s_hi >= 1) {
+                const int64_t g = gidx(x, y);
+                const bool odd = (s_hi & 1) != 0;
+                (odd ? p1 : p0)[g] = odd ? a1[r][k] : a0[r][k];
+                if (s_hi > s_lo) (odd ? p0 : p1)[g] = odd ? a0[r][k] : a1[r][k];
+            }
+        }
+    }
+}
+
+template <class T, int REGION, bool FOLD = true>
 __global__ void __launch_bounds__(32 * WARPS2D, sizeof(T) == 4 ? 2 : 1) swept2d_warp_kernel(T *__restrict__ p0, T *__restrict__ p1, int64_t nx, int64_t ny, int ox, int oy, int tiles_x, int64_t ntiles,
                                                                      typename Heat2D<T>::Consts c) {
     __shared__ T halo[WARPS2D][2][32];
@@ -245,8 +373,13 @@ __global__ void __launch_bounds__(32 * WARPS2D, sizeof(T) == 4 ? 2 : 1) swept2d_
     if (t >= ntiles * (REGION == R_BRIDGES ? 2 : 1)) return;
     // the two kinds of bridge are two instances of the tile code: with the kind a run-time value the compiler re-derived it (and
     // the rectangle) from the block and thread index inside every row group rather than spend registers on it
-    if (REGION == R_BRIDGES && t >= ntiles) tile32<T, REGION, true>(p0, p1, nx, ny, ox, oy, tiles_x, t - ntiles, halo[warp], lane, c);
-    else tile32<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, halo[warp], lane, c);
+    if constexpr (FOLD) {
+        if (REGION == R_BRIDGES && t >= ntiles) tile32f<T, REGION, true>(p0, p1, nx, ny, ox, oy, tiles_x, t - ntiles, halo[warp], lane, c);
+        else tile32f<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, halo[warp], lane, c);
+    } else {
+        if (REGION == R_BRIDGES && t >= ntiles) tile32<T, REGION, true>(p0, p1, nx, ny, ox, oy, tiles_x, t - ntiles, halo[warp], lane, c);
+        else tile32<T, REGION, false>(p0, p1, nx, ny, ox, oy, tiles_x, t, halo[warp], lane, c);
+    }
 }
 
 template <class T> typename Heat2D<T>::Consts consts_of(const swept2d_ctx *h) { return *reinterpret_cast<const typename Heat2D<T>::Consts *>(h->cb.bytes); }
@@ -282,7 +415,7 @@ template <class T, int W> cudaError_t sweep2d(swept2d_ctx *h, void *d_u, int64_t
     return cudaGetLastError();
 }
 
-template <class T> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K, cudaStream_t st, int64_t *launches) {
+template <class T, bool FOLD> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K, cudaStream_t st, int64_t *launches) {
     if (K <= 0) return cudaSuccess;
     constexpr int W = 32;
     T *p0 = (T *)d_u, *p1 = (T *)h->work;
@@ -290,20 +423,21 @@ template <class T> cudaError_t sweep2d_warp(swept2d_ctx *h, void *d_u, int64_t K
     const int64_t ntiles = (h->nx / W) * (h->ny / W);
     const dim3 block(32 * WARPS2D), grid((unsigned)((ntiles + WARPS2D - 1) / WARPS2D)), grid2((unsigned)((2 * ntiles + WARPS2D - 1) / WARPS2D));
     const typename Heat2D<T>::Consts c = consts_of<T>(h);
-    swept2d_warp_kernel<T, R_PYRAMID><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, 0, 0, tiles_x, ntiles, c);
+    swept2d_warp_kernel<T, R_PYRAMID, FOLD><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, 0, 0, tiles_x, ntiles, c);
     ++*launches;
     for (int64_t k = 0; k < K; ++k) {
         const int a = (int)(k & 1) * (W / 2), b = W / 2 - a;      // a: the alignment that shrinks in this half-cycle
-        swept2d_warp_kernel<T, R_BRIDGES><<<grid2, block, 0, st>>>(p0, p1, h->nx, h->ny, b, a, tiles_x, ntiles, c);
-        if (k == K - 1) swept2d_warp_kernel<T, R_INVERTED><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
-        else swept2d_warp_kernel<T, R_OCTAHEDRON><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
+        swept2d_warp_kernel<T, R_BRIDGES, FOLD><<<grid2, block, 0, st>>>(p0, p1, h->nx, h->ny, b, a, tiles_x, ntiles, c);
+        if (k == K - 1) swept2d_warp_kernel<T, R_INVERTED, FOLD><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
+        else swept2d_warp_kernel<T, R_OCTAHEDRON, FOLD><<<grid, block, 0, st>>>(p0, p1, h->nx, h->ny, b, b, tiles_x, ntiles, c);
         *launches += 2;
     }
     return cudaGetLastError();
 }
 
 template <class T> cudaError_t sweep2d_w(swept2d_ctx *h, void *d_u, int W, int64_t K, cudaStream_t st, int64_t *launches) {
-    if (W == 32 && h->kernel != SWEPT2D_KERNEL_SMEM) return sweep2d_warp<T>(h, d_u, K, st, launches);
+    if (W == 32 && h->kernel != SWEPT2D_KERNEL_SMEM)
+        return h->kernel == SWEPT2D_KERNEL_COLUMN ? sweep2d_warp<T, false>(h, d_u, K, st, launches) : sweep2d_warp<T, true>(h, d_u, K, st, launches);
     switch (W) {
         case 8: return sweep2d<T, 8>(h, d_u, K, st, launches);
         case 16: return sweep2d<T, 16>(h, d_u, K, st, launches);
@@ -390,7 +524,7 @@ extern "C" int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int ti
 
 extern "C" int swept2d_set_option(swept2d_handle_t h, int option, int value) {
     if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_set_option: NULL handle");
-    if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM))
+    if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM && value != SWEPT2D_KERNEL_COLUMN))
         return swept_fail(SWEPT_EINVAL, "swept2d_set_option: unknown option %d or value %d", option, value);
     h->kernel = value;
     return SWEPT_OK;

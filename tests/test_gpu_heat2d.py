@@ -10,7 +10,7 @@ from gpu_util import TOL, assert_bits_equal, rel_max, to_dev
 pytestmark = pytest.mark.gpu
 
 
-KERNELS = {"warp": sw.KERNEL2D_WARP, "smem": sw.KERNEL2D_SMEM}     # W = 32 only; narrower tiles always run on the shared-memory kernels
+KERNELS = {"warp": sw.KERNEL2D_WARP, "smem": sw.KERNEL2D_SMEM, "column": sw.KERNEL2D_COLUMN}     # W = 32 only; narrower tiles always run on the shared-memory kernels
 
 
 def _run(nx, ny, dtype, nsteps, W=None, fo=0.2, u0=None, kernel="warp"):
@@ -50,9 +50,9 @@ def test_classic_2d_matches_oracle(nx, ny, nsteps, dtype):
     (64, 32, 32, 16),        # one half-cycle: pyramid, bridges, inverted pyramid
     (32, 128, 32, 16 * 4 + 1),
 ])
-@pytest.mark.parametrize("kernel", ["warp", "smem"])
+@pytest.mark.parametrize("kernel", ["warp", "column", "smem"])
 def test_swept_2d_equals_classic_and_oracle(nx, ny, W, nsteps, dtype, kernel):
-    if kernel == "smem" and W != 32:
+    if kernel != "warp" and W != 32:
         pytest.skip("W < 32 has one kernel family")
     got, info = _run(nx, ny, dtype, nsteps, W=W, kernel=kernel)
     ref, _ = _run(nx, ny, dtype, nsteps)
@@ -74,8 +74,9 @@ def test_swept_2d_full_size_sampled_against_the_oracle():
     got, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0)
     ref, _ = _run(n, n, np.float64, nsteps, u0=u0)
     assert_bits_equal(got, ref, "swept 2-D (register kernel) vs classic at 4096^2")
-    smem, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0, kernel="smem")
-    assert_bits_equal(smem, ref, "swept 2-D (shared-memory kernel) vs classic at 4096^2")
+    for kern in ("column", "smem"):
+        other, _ = _run(n, n, np.float64, nsteps, W=32, u0=u0, kernel=kern)
+        assert_bits_equal(other, ref, f"swept 2-D ({kern} kernel) vs classic at 4096^2")
     dx, dt = wl.heat2d_grid(n, 0.2)
     for cy, cx in ((0, 0), (n // 2 + 16, n // 2 + 16)):
         iy, ix = (cy - M // 2 + np.arange(M)) % n, (cx - M // 2 + np.arange(M)) % n
@@ -109,11 +110,12 @@ def test_the_two_2d_kernels_agree():
     u0 = wl.heat2d_field(nx, ny)
     for K in (1, 2, 3):
         outs = []
-        for kern in ("warp", "smem"):
+        for kern in ("warp", "column", "smem"):
             with sw.Solver2D(nx, ny, dx, dt) as s:
                 s.set_option(sw.OPT2D_KERNEL, KERNELS[kern])
                 u = to_dev(u0)
                 s.swept_run(u, 16 * K, 32)
                 torch.cuda.synchronize()
                 outs.append(u.cpu().numpy())
-        assert_bits_equal(outs[0], outs[1], f"register vs shared-memory 2-D kernels, {K} half-cycles")
+        assert_bits_equal(outs[0], outs[1], f"folded vs column register kernels, {K} half-cycles")
+        assert_bits_equal(outs[0], outs[2], f"register vs shared-memory 2-D kernels, {K} half-cycles")
