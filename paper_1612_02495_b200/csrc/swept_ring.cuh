@@ -89,7 +89,10 @@ template <class P, int PW> constexpr int ring_nwmax() {
     warps = warps >= 4 ? (warps & ~3) : 4;
     return (warps > 28 ? 28 : warps) - 1;
 }
-template <class P, int PW> constexpr bool ring_has_roomy() { return ring_nwmax<P, PW>() > RING_ROOMY && 65536 / (32 * (ring_nwmax<P, PW>() + 1)) < (P::GROUPED ? 255 : 128); }
+// heat: up to 7 computing warps per SM (8 warps x 255 registers is still the whole register file) -- measured, W = 512: nx = 2^18 2849 -> 2993,
+// 2^19 3819 -> 4068 GPts*steps/s; KS W = 256 loses with 7 (2^17 210 -> 179) and keeps 3
+template <class P> constexpr int ring_roomy() { return P::H == 1 ? 7 : RING_ROOMY; }
+template <class P, int PW> constexpr bool ring_has_roomy() { return ring_nwmax<P, PW>() > ring_roomy<P>() && 65536 / (32 * (ring_nwmax<P, PW>() + 1)) < (P::GROUPED ? 255 : 128); }
 
 // Bands are dealt over the computing warps of the grid: band n -> warp (n mod (blocks x wpb)) / blocks of block n mod blocks, so
 // that neighbouring bands sit on different SMs and every warp owns floor or ceil(ntiles / (blocks x wpb)) of them (the BandGrid
@@ -636,7 +639,7 @@ cudaError_t wave_ring(void *u, void *w, int64_t nx, int64_t q, int rt, void *syn
     if constexpr (!RingGeom<P, PW>::OK) return cudaErrorNotSupported;
     else {
         if constexpr (ring_has_roomy<P, PW>()) {
-            if (nx / RingGeom<P, PW>::W <= (int64_t)RING_ROOMY * sm_count) return wave_ring_pw<P, PW, RING_ROOMY>(u, w, nx, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
+            if (nx / RingGeom<P, PW>::W <= (int64_t)ring_roomy<P>() * sm_count) return wave_ring_pw<P, PW, ring_roomy<P>()>(u, w, nx, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
         }
         return wave_ring_pw<P, PW, ring_nwmax<P, PW>()>(u, w, nx, q, rt, sync, cb, sm_count, max_smem, max_warps, st);
     }
@@ -645,7 +648,7 @@ template <class P, int PW> cudaError_t ring_prepare(int max_smem) {
     if constexpr (!RingGeom<P, PW>::OK) return cudaSuccess;
     else {
         if constexpr (ring_has_roomy<P, PW>()) {
-            cudaError_t e = ring_prepare_pw<P, PW, RING_ROOMY>(max_smem);
+            cudaError_t e = ring_prepare_pw<P, PW, ring_roomy<P>()>(max_smem);
             if (e != cudaSuccess) return e;
         }
         return ring_prepare_pw<P, PW, ring_nwmax<P, PW>()>(max_smem);
