@@ -120,6 +120,67 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
     using T = typename P::real;
     constexpr int H = P::H, NC = P::NC, D = 2 * H, NP = PW / D;
     T old[SR][D][NC];
+#ifndef BAND_HEAT_BREADTH_FIRST
+#define BAND_HEAT_BREADTH_FIRST 1
+#endif
+    if constexpr (BAND_HEAT_BREADTH_FIRST && !P::GROUPED && H == 1 && NC == 1 && P::S == 1) {
+        // Heat: the SR x D point updates of one step are independent (super-row s + 1 runs one point behind super-row s): all sums,
+        // then all products, then all fused multiply-adds, in that source order, so that a warp alone on its scheduler keeps SR D
+        // chains in flight instead of the two or three the point-by-point order left it (ncu, nx = 2^18: `wait` 1.25 per issue)
+#pragma unroll
+        for (int step = 0; step < NP + SR - 1; ++step) {
+            T t[SR][D], v[SR][D], o[SR][D];
+#pragma unroll
+            for (int s = 0; s < SR; ++s) {
+                const int n = step - s;
+                if (n == 0) {
+#pragma unroll
+                    for (int rho = 0; rho < D; ++rho) X[0][D - 1 - rho] = recv[s][0][rho];
+                }
+            }
+#pragma unroll
+            for (int s = 0; s < SR; ++s) {
+                const int n = step - s;
+                if (n < 0 || n >= NP) continue;
+#pragma unroll
+                for (int rho = 0; rho < D; ++rho) {
+                    const int qq = (D - 1 - rho) + D * n;
+                    t[s][rho] = X[0][qq + 2] + X[0][qq];
+                }
+            }
+#pragma unroll
+            for (int s = 0; s < SR; ++s) {
+                const int n = step - s;
+                if (n < 0 || n >= NP) continue;
+#pragma unroll
+                for (int rho = 0; rho < D; ++rho) v[s][rho] = c.c0 * X[0][(D - 1 - rho) + D * n + 1];
+            }
+#pragma unroll
+            for (int s = 0; s < SR; ++s) {
+                const int n = step - s;
+                if (n < 0 || n >= NP) continue;
+#pragma unroll
+                for (int rho = 0; rho < D; ++rho) o[s][rho] = fp<T>::fma(c.Fo, t[s][rho], v[s][rho]);
+            }
+#pragma unroll
+            for (int s = 0; s < SR; ++s) {
+                const int n = step - s;
+                if (n < 0 || n >= NP) continue;
+                const int tt = tb + s + n;
+                const bool pact = ALL ? true : (tt > lo && tt <= hi);
+#pragma unroll
+                for (int rho = 0; rho < D; ++rho) {
+                    const int qq = (D - 1 - rho) + D * n;
+                    X[0][qq + D] = pact ? o[s][rho] : X[0][qq + D];
+                }
+                if (n == NP - 1) {
+#pragma unroll
+                    for (int rho = 0; rho < D; ++rho) keep[s][0][rho] = X[0][PW + (D - 1 - rho)];
+                }
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int step = 0; step < NP + SR - 1; ++step) {
 #pragma unroll
