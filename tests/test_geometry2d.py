@@ -94,3 +94,63 @@ def test_region_volumes():
         du = sum(2 * s * (W - 2 * s) for s in range(1, L + 1))
         dd = sum((2 * s) ** 2 for s in range(1, L + 1))
         assert uu + 2 * du + dd == L * W * W
+
+
+# ---- the register kernels' closed forms (csrc/heat2d.cu: tile32, tile32f) -------------------------------------------------------
+def _rect(region, ybridge, s, W=32):
+    """The rectangle [xa, xb) x [ya, yb) a tile updates at local tier s, as the kernels compute it."""
+    L = C = W // 2
+    if region == "pyramid":
+        return s, W - s, s, W - s
+    if region == "bridges":
+        ea, eb, sa, sb = C - s, C + s, s, W - s
+        return (sa, sb, ea, eb) if ybridge else (ea, eb, sa, sb)
+    if s <= L:
+        return C - s, C + s, C - s, C + s
+    return s - L, W - (s - L), s - L, W - (s - L)
+
+
+REGIONS = [("pyramid", False, 15), ("bridges", False, 15), ("bridges", True, 15), ("inverted", False, 16), ("octahedron", False, 31)]
+
+
+@pytest.mark.parametrize("region,ybridge,S1", REGIONS)
+def test_register_kernel_store_rule_matches_the_rectangles(region, ybridge, S1):
+    """The register kernels do not record which tiers touched a point; they store by closed form: point (x, y) was updated at the
+    tiers [s_lo, s_hi] (none if s_hi < s_lo).  Brute force over the rectangles: the set of tiers is exactly that interval."""
+    W, L, C = 32, 16, 16
+    for y in range(W):
+        for x in range(W):
+            tiers = [s for s in range(1, S1 + 1) if (lambda r: r[0] <= x < r[1] and r[2] <= y < r[3])(_rect(region, ybridge, s))]
+            ux, uy = min(x, W - 1 - x), min(y, W - 1 - y)
+            dx, dy = max(C - x, x - C + 1), max(C - y, y - C + 1)
+            if region == "pyramid":
+                s_lo, s_hi = 1, min(ux, uy)
+            elif region == "bridges":
+                s_lo, s_hi = (dy, ux) if ybridge else (dx, uy)
+            elif region == "inverted":
+                s_lo, s_hi = max(dx, dy), L
+            else:
+                s_lo, s_hi = max(dx, dy), L + min(ux, uy)
+            want = list(range(s_lo, s_hi + 1)) if s_hi >= s_lo and s_hi >= 1 else []
+            assert tiers == want, (region, ybridge, x, y, tiers, want)
+
+
+@pytest.mark.parametrize("region,ybridge,S1", REGIONS)
+def test_folded_layout_of_the_register_kernel(region, ybridge, S1):
+    """tile32f folds rows 16..31 onto lanes 16..31 (register row r holds row r in the lower half, row 31 - r in the upper) and
+    runs register rows ya..15 of both halves together.  That needs (1) every rectangle symmetric about the centre row, yb = 32 - ya
+    with ya <= 15; (2) the row terms of the store rule equal in both halves: min(y, 31 - y) = r and max(16 - y, y - 15) = 16 - r;
+    (3) only the full-tile tier (s = L of an inverted pyramid) touching rows 0 / 31 and columns 0 / 31, the only places where the
+    fold's halo values are used."""
+    W, L = 32, 16
+    for s in range(1, S1 + 1):
+        xa, xb, ya, yb = _rect(region, ybridge, s)
+        if xa >= xb or ya >= yb:
+            assert region == "bridges" and s == L        # (a bridge's tier L would be empty; the kernels stop at L - 1)
+            continue
+        assert ya + yb == W and 0 <= ya <= 15
+        full = region in ("inverted", "octahedron") and s == L
+        assert (ya == 0) == full and (xa == 0 or xb == W) == full
+    for r in range(16):
+        for y in (r, 31 - r):
+            assert min(y, W - 1 - y) == r and max(16 - y, y - 15) == 16 - r
