@@ -147,6 +147,9 @@ typedef struct {
                                     blocks_per_sm_cap = 0 (0 = none); used while SWEPT_OPT_BLOCKS_PER_SM is 0          */
     int tuned_pack;              /* SWEPT_OPT_PACK value (1 | 2) swept_tune measured as faster for the tuned width and kernel;
                                     0 = not measured (not heat fp32 on the band kernel)                              */
+    int tuned_kernel;            /* -1, or SWEPT_KERNEL_SMEM where swept_tune -- under the default options -- measured the
+                                    paper-style shared-memory kernels as fastest: swept_run then runs the tuned width on them
+                                    (tuned_chain = 0).  Small Euler grids.                                           */
 } swept_info_t;
 
 /* Create a solver for `problem` on nx periodic points with spacing dx and timestep dt (the paper's
@@ -206,7 +209,9 @@ int swept_band_owner(const swept_band_layout_t *layout, int band, int *block, in
  * fastest in the handle and return it in *best_tile_width (may be NULL).  Under the default SWEPT_OPT_CHAIN = 3 each
  * width is timed with the ring kernel, the streaming band kernel and the tile-flag kernel, and swept_run uses the fastest of
  * the three for the tuned width; with blocks_per_sm_cap = 0 the register-resident per-tile kernels are also timed at 4, 3 and 2 blocks
- * of 4 warps per SM (the paper's occupancy trade-off).  SYNCHRONISES the stream. */
+ * of 4 warps per SM (the paper's occupancy trade-off), and the paper-style shared-memory kernels compete as
+ * well: where they win (small Euler grids) swept_run runs the tuned width on them (swept_info_t.tuned_kernel).  The returned width is
+ * then legal for that family, not necessarily for SWEPT_KERNEL_WAVE.  SYNCHRONISES the stream. */
 int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *best_tile_width, void *cuda_stream);
 
 /* End-to-end convenience used for the `e2e` measurement: copy h_u (HOST, [ncomp][nx], ideally

@@ -58,7 +58,7 @@ class _Info(ctypes.Structure):
         ("nx", ctypes.c_int64), ("workspace_bytes", ctypes.c_int64), ("tuned_tile_width", ctypes.c_int),
         ("launches_last_call", ctypes.c_int64), ("launches_total", ctypes.c_int64), ("sm_count", ctypes.c_int),
         ("max_smem_per_block", ctypes.c_int), ("last_sweep_launch", ctypes.c_int), ("boundary", ctypes.c_int), ("tuned_chain", ctypes.c_int), ("tuned_blocks_per_sm", ctypes.c_int),
-        ("tuned_pack", ctypes.c_int),
+        ("tuned_pack", ctypes.c_int), ("tuned_kernel", ctypes.c_int),
     ]
 
 

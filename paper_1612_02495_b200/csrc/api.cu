@@ -28,7 +28,7 @@ struct swept_ctx {
     unsigned *abort_seen;  // pinned host copy of the abort word, refreshed by an async copy behind every launch-free launch
     cudaEvent_t busy;      // recorded behind the work of every call; the next call's stream waits on it (calls on one handle
                            // from several streams are serialised on the device instead of corrupting the shared scratch)
-    int max_tile_width, tuned_tile_width, tuned_chain, tuned_cap, last_sweep_launch;   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
+    int max_tile_width, tuned_tile_width, tuned_chain, tuned_cap, tuned_kernel, last_sweep_launch;   // tuned_kernel: -1 = the option's family   // tuned_chain: 1 | 2 for tuned_tile_width, 0 = not tuned
     int64_t launches_last, launches_total;
     // cached CUDA graphs (one per path; rebuilt when the key changes)
     cudaGraphExec_t ngraph;  void *ngraph_u;  int64_t ngraph_steps, ngraph_launches;
@@ -126,6 +126,7 @@ extern "C" int swept_create(swept_handle_t *out, int problem, int64_t nx, double
     h->kernel = SWEPT_KERNEL_WAVE;
     h->chain = 3;
     h->last_sweep_launch = -1;
+    h->tuned_kernel = -1;
     h->warps_per_block = 4;
     h->max_tile_width = p ? p->max_tile_width : 0;
     if (dtype == SWEPT_F64) fill_consts<double>(h); else fill_consts<float>(h);
@@ -216,12 +217,20 @@ extern "C" int swept_tile_width_ok(swept_handle_t h, int tile_width) {
     return check_width(h, tile_width, h->kernel, true);
 }
 
+// The kernel family swept_run uses for width W: the option's, except that under the default options (register kernels, launch-free
+// sweep chosen by the tuner) the tuned width runs on the paper-style shared-memory kernels where swept_tune measured them faster
+// (Euler on grids that give a lane-per-8-cells kernel too few warps: nx <= 2^16).
+static int tuned_family(const swept_ctx *h, int W) {
+    if (h->kernel == SWEPT_KERNEL_WAVE && h->chain == 3 && h->tuned_kernel >= 0 && W == h->tuned_tile_width) return h->tuned_kernel;
+    return h->kernel;
+}
+
 // The width swept_run uses for tile_width = 0: the tuned one, else the largest legal width not above 256 (WAVE) / 512 (SMEM)
 // and nx.  Grids too small for the narrowest register tile (32 lanes x 2h points) fall back to the paper-style shared-memory
 // kernels, which take any power of two >= 4h: *kernel is the family to run.
 static int default_width(const swept_ctx *h, int *kernel) {
     *kernel = h->kernel;
-    if (h->tuned_tile_width) return h->tuned_tile_width;
+    if (h->tuned_tile_width) { *kernel = tuned_family(h, h->tuned_tile_width); return h->tuned_tile_width; }
     for (int W = h->kernel == SWEPT_KERNEL_WAVE ? 256 : 512; W >= 4 * h->H; W >>= 1)
         if (check_width(h, W, h->kernel, false)) return W;
     if (h->kernel == SWEPT_KERNEL_WAVE && !h->bc) {
@@ -502,7 +511,10 @@ extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_w
     if (W == 0) {
         W = default_width(h, &kernel);
         if (W == 0) return fail(SWEPT_EINVAL, "swept_run: no legal tile width for nx=%lld with the selected kernel", (long long)h->nx);
-    } else if (!check_width(h, W, h->kernel, true)) return SWEPT_EINVAL;
+    } else {
+        kernel = tuned_family(h, W);                      // the tuned width runs on the family the tuner measured as fastest
+        if (!check_width(h, W, kernel, true)) return SWEPT_EINVAL;
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = handle_enter(h, st, "swept_run"))) return rc;
     int64_t launches = 0;
@@ -555,6 +567,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     const int saved_chain = h->chain;
     h->tuned_chain = 0;
     h->tuned_cap = 0;
+    h->tuned_kernel = -1;
     const bool wave = h->kernel == SWEPT_KERNEL_WAVE;
     for (int W = 4 * h->H; W <= wtop && e == cudaSuccess; W <<= 1) {
         if (!check_width(h, W, h->kernel, false)) continue;
@@ -592,6 +605,31 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
         }
     }
     h->chain = saved_chain;
+    // default options: the paper-style shared-memory kernels compete too (one thread per point: on small Euler grids they have 8 x
+    // the parallelism of the register kernels' lane per 8 cells)
+    int best_kernel = -1;
+    // ... which can only matter while the grid gives the register kernels fewer than four warps per SM sub-partition at their
+    // narrowest launch-free tile (64 x 2h points); on larger grids the candidates would only cost tuning time
+    const bool few_warps = h->nx / (64 * 2 * h->H) < (int64_t)16 * h->sm_count;
+    if (wave && saved_chain == 3 && blocks_per_sm_cap == 0 && !h->bc && few_warps && e == cudaSuccess) {
+        h->blocks_per_sm = 0;
+        for (int W = 32; W <= wmax && e == cudaSuccess; W <<= 1) {
+            if (!check_width(h, W, SWEPT_KERNEL_SMEM, false)) continue;
+            float ms_min = 1e30f;
+            for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {
+                int64_t l = 0;
+                cudaEventRecord(e0, st);
+                e = enqueue_swept(h, SWEPT_KERNEL_SMEM, d_u_scratch, nsteps, W, st, &l);
+                cudaEventRecord(e1, st);
+                if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+                float ms = 0;
+                if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+                if (rep > 0 && ms < ms_min) ms_min = ms;
+                h->launches_total += l;
+            }
+            if (e == cudaSuccess && ms_min < best_ms) { best_ms = ms_min; best = W; best_chain = 0; best_cap = 0; best_pack = 0; best_kernel = SWEPT_KERNEL_SMEM; }
+        }
+    }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     h->blocks_per_sm = saved_cap;
@@ -603,6 +641,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     h->tuned_chain = (saved_chain == 3 && h->kernel == SWEPT_KERNEL_WAVE) ? best_chain : 0;
     h->tuned_cap = blocks_per_sm_cap == 0 ? best_cap : 0;
     h->tuned_pack = best_pack;
+    h->tuned_kernel = best_kernel;
     if (best_tile_width) *best_tile_width = best;
     return SWEPT_OK;
 }
@@ -636,7 +675,7 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
     switch (key) {
         case SWEPT_OPT_KERNEL:
             if (value != SWEPT_KERNEL_SMEM && value != SWEPT_KERNEL_WAVE) return fail(SWEPT_EINVAL, "swept_set_option: unknown kernel %d", value);
-            if (value != h->kernel) { h->tuned_tile_width = 0; h->tuned_chain = 0; h->tuned_cap = 0; }
+            if (value != h->kernel) { h->tuned_tile_width = 0; h->tuned_chain = 0; h->tuned_cap = 0; h->tuned_kernel = -1; }
             h->kernel = value;
             return SWEPT_OK;
         case SWEPT_OPT_NAIVE_GRAPH:
@@ -687,6 +726,7 @@ extern "C" int swept_get_info(swept_handle_t h, swept_info_t *info) {
     info->tuned_chain = h->tuned_chain;
     info->tuned_blocks_per_sm = h->tuned_cap;
     info->tuned_pack = h->tuned_pack;
+    info->tuned_kernel = h->tuned_kernel;
     return SWEPT_OK;
 }
 

@@ -383,9 +383,44 @@ def test_tuner_chooses_between_bands_and_tile_flags():
     with solver_for(w, np.float64) as s:
         W = s.tune(to_dev(w.initial(np.float64)))
         info = s.info()
-        assert info["tuned_tile_width"] == W and info["tuned_chain"] in (sw.CHAIN_TILES, sw.CHAIN_BANDS, sw.CHAIN_RING)
+        assert info["tuned_tile_width"] == W
         nsteps = 7 * _sph(wl.EULER, W) + 1
-        assert_bits_equal(run_swept(w, np.float64, nsteps, W, (sw.KERNEL_WAVE, info["tuned_chain"])), run_naive(w, np.float64, nsteps), "tuned variant")
+        if info["tuned_kernel"] == sw.KERNEL_SMEM:      # small Euler grids: the paper-style kernels (a thread per cell) can win
+            assert info["tuned_chain"] == 0
+            variant = (sw.KERNEL_SMEM, sw.CHAIN_OFF)
+        else:
+            assert info["tuned_kernel"] == -1 and info["tuned_chain"] in (sw.CHAIN_TILES, sw.CHAIN_BANDS, sw.CHAIN_RING)
+            variant = (sw.KERNEL_WAVE, info["tuned_chain"])
+        assert_bits_equal(run_swept(w, np.float64, nsteps, W, variant), run_naive(w, np.float64, nsteps), "tuned variant")
+        # the default run (tile_width 0, and the tuned width given explicitly) uses what the tuner chose
+        import torch
+        for tw in (0, W):
+            u = to_dev(w.initial(np.float64))
+            s.swept_run(u, nsteps, tw)
+            torch.cuda.synchronize()
+            assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float64, nsteps), f"default run after tune, tile_width={tw}")
+            ran = s.info()["last_sweep_launch"]
+            assert (ran == sw.LAUNCH_DIAMOND) == (info["tuned_kernel"] == sw.KERNEL_SMEM)
+
+
+def test_tuner_picks_the_shared_memory_kernels_for_a_small_euler_grid():
+    """nx = 2^12 Euler: 16 tiles of 256 cells give the register kernels 16 warps of 8 cells per lane; the paper-style kernels run a
+    thread per cell.  The tuner measures both families under the default options and swept_run follows it."""
+    import torch
+    w = _noise(wl.EULER, 1 << 12)
+    with solver_for(w, np.float64) as s:
+        W = s.tune(to_dev(w.initial(np.float64)))
+        info = s.info()
+        assert info["tuned_kernel"] == sw.KERNEL_SMEM and info["tuned_chain"] == 0 and info["tuned_tile_width"] == W
+        u = to_dev(w.initial(np.float64))
+        s.swept_run(u, 301, 0)
+        torch.cuda.synchronize()
+        assert s.info()["last_sweep_launch"] == sw.LAUNCH_DIAMOND
+        assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float64, 301), "tuned shared-memory run")
+        s.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)       # an explicit choice of kernel overrides the tuner's family
+        s.swept_run(u, 64, 256)
+        torch.cuda.synchronize()
+        assert s.info()["last_sweep_launch"] != sw.LAUNCH_DIAMOND
 
 
 # ------------------------------------------------------------------------------------------------------------
