@@ -119,3 +119,24 @@ def test_the_two_2d_kernels_agree():
                 outs.append(u.cpu().numpy())
         assert_bits_equal(outs[0], outs[1], f"folded vs column register kernels, {K} half-cycles")
         assert_bits_equal(outs[0], outs[2], f"register vs shared-memory 2-D kernels, {K} half-cycles")
+
+
+def test_random_2d_configurations_match_the_classic_path_bitwise():
+    """Seeded random (nx, ny, tile width, kernel, step count, dtype): swept == classic bit for bit."""
+    import torch
+    rng = np.random.default_rng(2495)
+    ran = 0
+    for _ in range(60):
+        nx, ny = (1 << int(rng.integers(3, 10))), (1 << int(rng.integers(3, 10)))
+        W = int(rng.choice([8, 16, 32]))
+        kern = str(rng.choice(["warp", "column", "smem"]))
+        dtype = np.float64 if rng.random() < 0.5 else np.float32
+        nsteps = int(rng.integers(1, 5 * W))
+        if W > min(nx, ny):
+            continue
+        u0 = rng.uniform(-1, 1, (ny, nx)).astype(dtype)
+        got, _ = _run(nx, ny, dtype, nsteps, W=W, u0=u0, kernel=kern)
+        ref, _ = _run(nx, ny, dtype, nsteps, u0=u0)
+        assert_bits_equal(got, ref, f"2-D {nx}x{ny} W={W} {kern} {np.dtype(dtype).name} nsteps={nsteps}")
+        ran += 1
+    assert ran >= 30
