@@ -75,6 +75,10 @@ enum {
                                      block per SM, caps its warps at 4 x this), 0 = none / the tuner's choice        */
     SWEPT_OPT_WARPS_PER_BLOCK = 3,/* WAVE kernels: lane groups are packed this many warps a block   */
     SWEPT_OPT_SWEPT_GRAPH = 4,    /* 1: swept_run replays a CUDA graph of its half-cycle launches  */
+    SWEPT_OPT_NAIVE_SHARE = 7,    /* Euler, classic path: 1 = a thread evaluates the faces between the 2 (fp64) / 4 (fp32) cells it updates
+                                     once (3 / 5 face fluxes instead of 4 / 8): the same operations on the same operands, bit-identical.
+                                     Default 0: every point through the per-point stencil function, the paper's naive kernel (Fig. 6).
+                                     Ignored for heat and KS                                                            */
     SWEPT_OPT_PACK = 6,           /* heat fp32 on the streaming band kernel: 2 = every warp slot advances TWO bands (half a domain
                                      apart) in lock step on packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: half the FP
                                      instructions, per-component IEEE rounding, so the result is bit-identical); 1 = one band

@@ -18,7 +18,7 @@ from typing import Optional
 HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
-OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN, OPT_PACK = 0, 1, 2, 3, 4, 5, 6
+OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN, OPT_PACK, OPT_NAIVE_SHARE = 0, 1, 2, 3, 4, 5, 6, 7
 PACK_AUTO, PACK_OFF, PACK_ON = 0, 1, 2
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}

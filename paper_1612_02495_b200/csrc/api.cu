@@ -22,7 +22,7 @@ struct swept_ctx {
     size_t field_bytes;    // NC*nx*sizeof(T)
     void *host_stage;      // device buffer for swept_run_host (allocated on first use)
     int device, sm_count, max_smem;
-    int kernel, chain, naive_graph, swept_graph, blocks_per_sm, warps_per_block, pack, tuned_pack;
+    int kernel, chain, naive_graph, naive_share, swept_graph, blocks_per_sm, warps_per_block, pack, tuned_pack;
     void *sync_base;       // SYNC_HEADER bytes (word 0: the abort word of the bounded waits, swept_wave.cuh) + the sync area
     void *sync;            // sync area = sync_base + SYNC_HEADER; chain kernel: work counter (8 bytes) + done[] flags; band kernel: prog[]
     unsigned *abort_seen;  // pinned host copy of the abort word, refreshed by an async copy behind every launch-free launch
@@ -280,7 +280,7 @@ static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cuda
     if (h->S == 1) {
         void *a = d_u, *b = h->work;
         for (int64_t m = 0; m < nsteps; ++m) {
-            e = launch_classic_stage(h->problem, h->dtype, 1, a, a, b, h->nx, h->cb, h->bc, st);
+            e = launch_classic_stage(h->problem, h->dtype, 1, a, a, b, h->nx, h->cb, h->bc, h->naive_share, st);
             if (e != cudaSuccess) return e;
             void *t = a; a = b; b = t;
             ++*launches;
@@ -290,9 +290,9 @@ static cudaError_t enqueue_classic(swept_ctx *h, void *d_u, int64_t nsteps, cuda
         }
     } else {
         for (int64_t m = 0; m < nsteps; ++m) {
-            e = launch_classic_stage(h->problem, h->dtype, 1, d_u, d_u, h->work, h->nx, h->cb, h->bc, st);
+            e = launch_classic_stage(h->problem, h->dtype, 1, d_u, d_u, h->work, h->nx, h->cb, h->bc, h->naive_share, st);
             if (e != cudaSuccess) return e;
-            e = launch_classic_stage(h->problem, h->dtype, 0, h->work, d_u, d_u, h->nx, h->cb, h->bc, st);
+            e = launch_classic_stage(h->problem, h->dtype, 0, h->work, d_u, d_u, h->nx, h->cb, h->bc, h->naive_share, st);
             if (e != cudaSuccess) return e;
             *launches += 2;
         }
@@ -681,6 +681,11 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
         case SWEPT_OPT_NAIVE_GRAPH:
             if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: NAIVE_GRAPH takes 0 or 1");
             h->naive_graph = value;
+            return SWEPT_OK;
+        case SWEPT_OPT_NAIVE_SHARE:
+            if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: NAIVE_SHARE takes 0 or 1");
+            if (value != h->naive_share) drop_graphs(h);
+            h->naive_share = value;
             return SWEPT_OK;
         case SWEPT_OPT_SWEPT_GRAPH:
             if (value != 0 && value != 1) return fail(SWEPT_EINVAL, "swept_set_option: SWEPT_GRAPH takes 0 or 1");

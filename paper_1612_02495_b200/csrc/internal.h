@@ -23,8 +23,9 @@ constexpr int SYNC_HEADER = 16;
 // One classic sub-timestep over all nx points (naive.cu).  odd: predictor stage of a two-stage scheme.
 // dst[i] = stage(win_src[i-H..i+H], base[i]); base may alias dst.
 // bc: SWEPT_BC_PERIODIC | SWEPT_BC_INSULATED (heat only: ghost value = adjacent interior value).
+// share: Euler only -- the faces between the cells one thread updates are evaluated once (SWEPT_OPT_NAIVE_SHARE).
 cudaError_t launch_classic_stage(int problem, int dtype, int odd, const void *win_src, const void *base, void *dst,
-                                 int64_t nx, const ConstBlock &cb, int bc, cudaStream_t st);
+                                 int64_t nx, const ConstBlock &cb, int bc, int share, cudaStream_t st);
 
 // Paper-style shared-memory swept kernels (swept_smem.cu): one block per tile of W points.
 // mode: MODE_UP | MODE_DIAMOND | MODE_DOWN; offset: tile-grid shift (0 or W/2).

@@ -22,7 +22,7 @@ template <bool INS> __device__ __forceinline__ int64_t classic_index(int64_t g, 
     return g & (nx - 1);
 }
 
-template <class P, bool ODD, bool INS = false>
+template <class P, bool ODD, bool INS = false, bool SHARE = false>
 __global__ void __launch_bounds__(256) classic_kernel(const typename P::real *__restrict__ src, const typename P::real *base,
                                                        typename P::real *dst, int64_t nx, typename P::Consts c) {
     using T = typename P::real;
@@ -52,6 +52,15 @@ __global__ void __launch_bounds__(256) classic_kernel(const typename P::real *__
             for (int j = 0; j < V; ++j) b[k][j] = T(0);
         }
     }
+    if constexpr (SHARE && P::GROUPED) {
+        // SWEPT_OPT_NAIVE_SHARE: the faces between the thread's V cells are evaluated once (V + 1 faces instead of 2 V)
+        T bb[V][NC];
+#pragma unroll
+        for (int j = 0; j < V; ++j)
+#pragma unroll
+            for (int k = 0; k < NC; ++k) bb[j][k] = b[k][j];
+        P::template cells<V>(c, ODD, w, bb, out);
+    } else {
 #pragma unroll
     for (int j = 0; j < V; ++j) {
         T win[NC][2 * H + 1], bb[NC];
@@ -62,6 +71,7 @@ __global__ void __launch_bounds__(256) classic_kernel(const typename P::real *__
             bb[k] = b[k][j];
         }
         P::template stage<ODD>(c, win, bb, out[j]);
+    }
     }
 #pragma unroll
     for (int k = 0; k < NC; ++k) {
@@ -74,7 +84,7 @@ __global__ void __launch_bounds__(256) classic_kernel(const typename P::real *__
 }
 
 template <class P>
-static cudaError_t launch_classic(int odd, const void *src, const void *base, void *dst, int64_t nx, const ConstBlock &cb, int bc,
+static cudaError_t launch_classic(int odd, const void *src, const void *base, void *dst, int64_t nx, const ConstBlock &cb, int bc, int share,
                                   cudaStream_t st) {
     using T = typename P::real;
     const typename P::Consts c = *reinterpret_cast<const typename P::Consts *>(cb.bytes);
@@ -89,15 +99,22 @@ static cudaError_t launch_classic(int odd, const void *src, const void *base, vo
             return cudaErrorNotSupported;
         }
     }
+    if constexpr (P::GROUPED) {
+        if (share) {
+            if (odd) classic_kernel<P, true, false, true><<<blocks, tpb, 0, st>>>((const T *)src, (const T *)base, (T *)dst, nx, c);
+            else     classic_kernel<P, false, false, true><<<blocks, tpb, 0, st>>>((const T *)src, (const T *)base, (T *)dst, nx, c);
+            return cudaGetLastError();
+        }
+    }
     if (odd) classic_kernel<P, true><<<blocks, tpb, 0, st>>>((const T *)src, (const T *)base, (T *)dst, nx, c);
     else     classic_kernel<P, false><<<blocks, tpb, 0, st>>>((const T *)src, (const T *)base, (T *)dst, nx, c);
     return cudaGetLastError();
 }
 
 cudaError_t launch_classic_stage(int problem, int dtype, int odd, const void *win_src, const void *base, void *dst, int64_t nx,
-                                 const ConstBlock &cb, int bc, cudaStream_t st) {
+                                 const ConstBlock &cb, int bc, int share, cudaStream_t st) {
     cudaError_t e = cudaSuccess;
-    SWEPT_DISPATCH(problem, dtype, P, e = launch_classic<P>(odd, win_src, base, dst, nx, cb, bc, st));
+    SWEPT_DISPATCH(problem, dtype, P, e = launch_classic<P>(odd, win_src, base, dst, nx, cb, bc, share, st));
     return e;
 }
 

@@ -220,6 +220,34 @@ def test_tuner_returns_a_legal_width_and_default_run_uses_it(kernel):
         assert_bits_equal(u.cpu().numpy(), run_naive(w, np.float32, 777), "tuned width run")
 
 
+@pytest.mark.parametrize("dtype", [np.float64, np.float32], ids=["f64", "f32"])
+def test_classic_euler_with_shared_faces_is_bit_identical(dtype):
+    """SWEPT_OPT_NAIVE_SHARE: the classic kernel evaluates the faces between a thread's cells once.  Same bits as the per-point
+    kernel and the oracle -- plain launches, graph replay, and as the remainder steps of a swept run."""
+    import torch
+    w = _noise(wl.EULER, 1 << 12)
+    nsteps = 137
+    ref = run_naive(w, dtype, nsteps)
+    assert_bits_equal(ref, run_oracle(w, dtype, nsteps), "per-point classic vs oracle")
+    for graph in (0, 1):
+        with solver_for(w, dtype) as s:
+            s.set_option(sw.OPT_NAIVE_SHARE, 1)
+            s.set_option(sw.OPT_NAIVE_GRAPH, graph)
+            u = to_dev(w.initial(dtype))
+            s.naive_run(u, nsteps)
+            torch.cuda.synchronize()
+            assert_bits_equal(u.cpu().numpy(), ref, f"shared-face classic (graph={graph}) vs per-point classic")
+            u = to_dev(w.initial(dtype))
+            s.set_option(sw.OPT_CHAIN, sw.CHAIN_TILES)
+            s.swept_run(u, nsteps, 256)              # 137 = 4 x 32 + 9: the remainder's classic steps take the option too
+            torch.cuda.synchronize()
+            assert_bits_equal(u.cpu().numpy(), ref, "swept run with shared-face remainder steps")
+    with solver_for(_noise(wl.HEAT, 1 << 10), np.float64) as s:
+        s.set_option(sw.OPT_NAIVE_SHARE, 1)           # accepted and ignored
+        with pytest.raises(sw.SweptError):
+            s.set_option(sw.OPT_NAIVE_SHARE, 2)
+
+
 def test_alu_peak_microbenchmark_is_plausible():
     p64 = sw.measure_alu_peak(sw.F64)["instr_per_s"]
     p32 = sw.measure_alu_peak(sw.F32)["instr_per_s"]
