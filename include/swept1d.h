@@ -223,6 +223,44 @@ int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm_cap, int *
  * result back into h_u, and synchronise the stream. */
 int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int tile_width, int use_swept, void *cuda_stream);
 
+/* The swept rule without a handle and without any allocation -- for callers that cannot call cudaMalloc.
+ *
+ * Who that is: a host program that gave the whole GPU to its own pool (a framework's caching allocator, a simulation code's
+ * arena, a fixed per-tenant budget), where a cudaMalloc from inside a library fails or eats into somebody else's share; a
+ * time-critical loop, where cudaMalloc / cudaFree stall the device for every stream; and code that runs where the CUDA
+ * runtime does not accept allocation calls at all.  swept_create needs three allocations (the odd-tier edge row R1, the flag
+ * area of the launch-free kernels, a pinned word), so none of these callers can have a handle.
+ *
+ * swept_run_static advances the caller's field d_u (DEVICE, [ncomp][nx], 16-byte aligned, caller-owned, updated in place) by
+ * nsteps timesteps exactly as swept_run does with SWEPT_OPT_KERNEL = SWEPT_KERNEL_WAVE and SWEPT_OPT_CHAIN = 0: the
+ * register-resident tile kernels, one launch per half-cycle -- upright triangle, diamonds on tiles
+ * shifted by W/2, closing inverted triangle -- with the nsteps mod (L/S) remaining timesteps first, on narrower tiles and the
+ * classic kernel (reading S3).  The result is bit-identical to swept_run and naive_run.  The odd-tier edges (the
+ * paper's left / right arrays), for which a handle owns a workspace, go through a fixed array of
+ * SWEPT_STATIC_SCRATCH_BYTES that is part of the library image: every GPU that loads the library holds these bytes until
+ * the process ends, whether or not this function is ever called.
+ *
+ *   problem, nx, dx, dt, p   as for swept_create (p may be NULL = f64, alpha 1, gamma 1.4); periodic domains only
+ *   tile_width               as for swept_run with the WAVE kernels; 0 = the widest legal width <= 256
+ *   cuda_stream              the work is only enqueued, as by swept_run
+ *
+ * Limit: ncomp * nx * sizeof(dtype) <= SWEPT_STATIC_SCRATCH_BYTES (heat / KS: nx <= 2^20 in fp64, 2^21 in fp32; Euler:
+ * nx <= 2^18 / 2^19); a larger field is refused with SWEPT_EINVAL before anything is enqueued.  Other errors as for swept_run.
+ * The call makes no cudaMalloc, cudaFree or other allocating call, creates no stream, event or graph, and never synchronises.
+ *
+ * First call on a device: the library looks up the device address of the array (cudaGetSymbolAddress -- in host code the
+ * array's own name is not a device pointer) and raises the shared-memory limits of the kernels for (problem, dtype); the
+ * device that is current at the call is the one set up and used.  Make that first call for each (device, problem, dtype)
+ * outside any stream capture.
+ *
+ * All calls on one device share the one array, and it keeps what the last call left there.  Nothing in it has to start
+ * at zero: every phase writes each odd-tier edge value before a later phase of the same call reads it, so old contents are
+ * never read.  But two calls whose kernels can overlap on the GPU (different streams, no ordering between them) race on the
+ * array and corrupt each other's edges: order them, or give all but one a handle. */
+#define SWEPT_STATIC_SCRATCH_BYTES (8 << 20)
+int swept_run_static(int problem, int64_t nx, double dx, double dt, const swept_params_t *p, void *d_u, int64_t nsteps,
+                     int tile_width, void *cuda_stream);
+
 /* Set a SWEPT_OPT_* option.  SWEPT_EINVAL for unknown keys / values. */
 int swept_set_option(swept_handle_t h, int key, int value);
 

@@ -33,6 +33,7 @@ SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
     "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak", "swept_measure_latencies",
+    "swept_run_static",
     # include/swept2d.h
     "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy",
 )
@@ -104,6 +105,7 @@ def lib() -> ctypes.CDLL:
     L.naive_run.argtypes = [vp, vp, i64, vp]
     L.swept_tune.argtypes = [vp, vp, ci, ctypes.POINTER(ci), vp]
     L.swept_run_host.argtypes = [vp, vp, i64, ci, ci, vp]
+    L.swept_run_static.argtypes = [ci, i64, dbl, dbl, ctypes.POINTER(_Params), vp, i64, ci, vp]
     L.swept_set_option.argtypes = [vp, ci, ci]
     L.swept_get_info.argtypes = [vp, ctypes.POINTER(_Info)]
     L.swept_tile_width_ok.argtypes = [vp, ci]
@@ -294,6 +296,33 @@ class Solver2D:
             self.close()
         except Exception:
             pass
+
+
+STATIC_SCRATCH_BYTES = 8 << 20      # SWEPT_STATIC_SCRATCH_BYTES (include/swept1d.h)
+
+
+def swept_run_static(problem, u, nsteps: int, dx: float, dt: float, *, tile_width: int = 0, alpha: float = 1.0, gamma: float = 1.4,
+                     stream=None) -> None:
+    """`swept_run_static` (include/swept1d.h): advance `u` -- a contiguous CUDA tensor of shape [ncomp, nx] (or [nx]), float64 or
+    float32 -- IN PLACE by `nsteps` timesteps with the swept rule, without a Solver and without any device allocation by the
+    library.  For programs that cannot let a library call cudaMalloc: the GPU's memory belongs to their own pool, or an
+    allocation's device-wide stall is not affordable where they call from.  The edge row a Solver would allocate is a fixed
+    array inside the library (STATIC_SCRATCH_BYTES), so the field may hold at most that many bytes; calls on one device share the
+    array and must not overlap on the GPU.  The first call per (device, problem, dtype) does a one-off set-up and belongs outside
+    stream capture.  Same bits as Solver.swept_run / naive_run."""
+    import torch
+    if isinstance(problem, str):
+        problem = PROBLEMS[problem]
+    if not (isinstance(u, torch.Tensor) and u.is_cuda and u.is_contiguous() and u.dtype in (torch.float64, torch.float32)):
+        raise SweptError(EINVAL, "u must be a contiguous CUDA tensor of dtype float64 or float32")
+    if u.device.index != torch.cuda.current_device():
+        raise SweptError(EINVAL, f"u lives on cuda:{u.device.index} but cuda:{torch.cuda.current_device()} is current")
+    ncomp = problem_info(int(problem))["ncomp"]
+    if u.numel() % ncomp:
+        raise SweptError(EINVAL, f"u must hold ncomp = {ncomp} rows")
+    p = _Params(_dtype_id(u.dtype), float(alpha), float(gamma), 0, BC_PERIODIC)
+    _check(lib().swept_run_static(int(problem), u.numel() // ncomp, float(dx), float(dt), ctypes.byref(p), u.data_ptr(), int(nsteps),
+                                  int(tile_width), _stream_ptr(stream)))
 
 
 def measure_alu_peak(dtype=F64, stream=None) -> dict:

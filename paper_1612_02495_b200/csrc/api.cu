@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 
 #include "internal.h"
@@ -790,5 +791,107 @@ extern "C" int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cu
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     e = run_smem_peak(sms, bytes_per_s, ms, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return fail_cuda(e, "swept_measure_smem_peak");
+    return SWEPT_OK;
+}
+
+// ---- swept_run_static: the swept rule for callers that must not allocate (include/swept1d.h) ------------------------
+// Row R1 of the staircase (the handle's `work`) lives in this file-scope array instead of a cudaMalloc'ed buffer.  Every
+// device that loads the library carries the array until the process exits.
+static __device__ __align__(256) unsigned char g_static_r1[SWEPT_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDevice {
+    void *r1;                    // DEVICE address of g_static_r1 on this device; nullptr until the set-up ran
+    unsigned char prepared[3][2];// kernel attributes set for (problem, dtype)
+    int sm_count, max_smem;
+};
+StaticDevice g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+}  // namespace
+
+// Once per device, with that device current.  In host code `g_static_r1` names a host-side shadow of the symbol, not device
+// memory: the address a kernel may use has to be asked for.
+static int static_setup(int dev, int problem, int dtype, StaticDevice **out) {
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(SWEPT_EINVAL, "swept_run_static: device ordinal %d outside [0, %d)", dev, STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice *d = &g_static_dev[dev];
+    if (!d->r1) {
+        void *p = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&p, g_static_r1);
+        if (e != cudaSuccess) return fail_cuda(e, "swept_run_static: cudaGetSymbolAddress(static scratch)");
+        if (!p || ((uintptr_t)p & 255) != 0) return fail(SWEPT_ECUDA, "swept_run_static: static scratch address %p is not 256-byte aligned", p);
+        e = cudaDeviceGetAttribute(&d->sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&d->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (e != cudaSuccess) return fail_cuda(e, "swept_run_static: device attributes");
+        d->r1 = p;
+    }
+    if (!d->prepared[problem][dtype]) {
+        const cudaError_t e = swept_wave_prepare(problem, dtype);    // cudaFuncSetAttribute only
+        if (e != cudaSuccess) return fail_cuda(e, "swept_run_static: kernel attribute setup");
+        d->prepared[problem][dtype] = 1;
+    }
+    *out = d;
+    return SWEPT_OK;
+}
+
+extern "C" int swept_run_static(int problem, int64_t nx, double dx, double dt, const swept_params_t *p, void *d_u, int64_t nsteps,
+                                int tile_width, void *cuda_stream) {
+    g_err[0] = 0;
+    if (problem != SWEPT_HEAT && problem != SWEPT_KS && problem != SWEPT_EULER) return fail(SWEPT_EINVAL, "swept_run_static: unknown problem %d", problem);
+    const int dtype = p ? p->dtype : SWEPT_F64;
+    if (dtype != SWEPT_F32 && dtype != SWEPT_F64) return fail(SWEPT_EINVAL, "swept_run_static: unknown dtype %d", dtype);
+    if (!is_pow2(nx) || nx < 8) return fail(SWEPT_EINVAL, "swept_run_static: nx=%lld must be a power of two >= 8", (long long)nx);
+    if (!isfinite(dx) || !isfinite(dt) || dx <= 0.0 || dt <= 0.0) return fail(SWEPT_EINVAL, "swept_run_static: dx and dt must be finite and positive");
+    const double alpha = p ? p->alpha : 1.0, gamma = p ? p->gamma : 1.4;
+    if (problem == SWEPT_HEAT && !(isfinite(alpha) && alpha > 0.0)) return fail(SWEPT_EINVAL, "swept_run_static: alpha must be finite and positive");
+    if (problem == SWEPT_EULER && !(isfinite(gamma) && gamma > 1.0)) return fail(SWEPT_EINVAL, "swept_run_static: gamma must be finite and > 1");
+    if (p && p->boundary != SWEPT_BC_PERIODIC) return fail(SWEPT_EINVAL, "swept_run_static: periodic domains only");
+    // the size limit comes before anything touches the device
+    const int NC = ncomp_of(problem);
+    if (nx > (int64_t)(SWEPT_STATIC_SCRATCH_BYTES / (NC * elem_size(dtype))))
+        return fail(SWEPT_EINVAL, "swept_run_static: the field has %lld x %d elements of %zu bytes, the static scratch holds %d bytes "
+                                  "(SWEPT_STATIC_SCRATCH_BYTES); larger grids need a handle (swept_create)",
+                    (long long)nx, NC, elem_size(dtype), (int)SWEPT_STATIC_SCRATCH_BYTES);
+
+    // a handle on the stack whose workspace is the static array: the host driver below is the one swept_run uses
+    swept_ctx ctx;
+    memset(&ctx, 0, sizeof ctx);
+    swept_ctx *h = &ctx;
+    h->problem = problem; h->dtype = dtype;
+    h->H = radius_of(problem); h->S = stages_of(problem); h->NC = NC;
+    h->nx = nx; h->dx = dx; h->dt = dt; h->alpha = alpha; h->gamma = gamma;
+    h->bc = SWEPT_BC_PERIODIC;
+    h->kernel = SWEPT_KERNEL_WAVE;
+    h->chain = 0;                          // one launch per half-cycle: needs no flags, no counters, no pinned abort word
+    h->last_sweep_launch = -1;
+    h->tuned_kernel = -1;
+    h->warps_per_block = 4;
+    h->field_bytes = (size_t)NC * (size_t)nx * elem_size(dtype);
+    if (dtype == SWEPT_F64) fill_consts<double>(h); else fill_consts<float>(h);
+    int rc = run_args_ok(h, d_u, nsteps, "swept_run_static");
+    if (rc) return rc;
+
+    int W = tile_width;
+    if (W == 0) {
+        for (int w = 256; w >= 4 * h->H && !W; w >>= 1)
+            if ((int64_t)w <= nx && swept_wave_supports(problem, dtype, w)) W = w;
+        if (!W) return fail(SWEPT_EINVAL, "swept_run_static: nx=%lld is narrower than the narrowest register-resident tile", (long long)nx);
+    }
+    char buf[160];
+    const char *why = width_problem(problem, dtype, nx, W, SWEPT_KERNEL_WAVE, 0, buf, sizeof buf);
+    if (why) return fail(SWEPT_EINVAL, "swept_run_static: tile_width %d: %s", W, why);
+
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_run_static: no CUDA device (this library has no CPU fallback)");
+    StaticDevice *sd = nullptr;
+    if ((rc = static_setup(dev, problem, dtype, &sd))) return rc;
+    h->device = dev; h->sm_count = sd->sm_count; h->max_smem = sd->max_smem;
+    h->work = sd->r1;
+
+    int64_t launches = 0;
+    e = enqueue_swept(h, SWEPT_KERNEL_WAVE, d_u, nsteps, W, (cudaStream_t)cuda_stream, &launches, 0);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_run_static");
     return SWEPT_OK;
 }
