@@ -28,8 +28,12 @@
  *     independent and run concurrently on different streams.  (A call made inside the caller's own stream capture skips
  *     that wait; the caller's graph must then order the handle's uses itself.)
  *   - The launch-free kernels wait on flags other warps of the same launch publish; every such wait is bounded (seconds).
- *     A wait that gives up makes the kernel exit, and the next call on the handle returns SWEPT_ECUDA once: the field that
- *     launch ran on is invalid.
+ *     A wait that gives up makes the kernel exit and marks the handle: the field that launch ran on is invalid, and so is the
+ *     result of every sweep enqueued on the handle behind it, until the mark is reported.  It is reported ONCE, as SWEPT_ECUDA,
+ *     by swept_check(h) (which waits for the handle's work), by swept_run_host (which synchronises anyway), or by the first
+ *     swept_run / naive_run / swept_tune on the handle that is called after the marked launch has finished on the device; a call
+ *     made while it is still running cannot know yet.  Reporting clears the mark: the handle works again.  A caller that
+ *     synchronises its own stream and reads d_u without another handle call should call swept_check first.
  */
 #ifndef SWEPT1D_H
 #define SWEPT1D_H
@@ -79,6 +83,9 @@ enum {
                                      once (3 / 5 face fluxes instead of 4 / 8): the same operations on the same operands, bit-identical.
                                      Default 0: every point through the per-point stencil function, the paper's naive kernel (Fig. 6).
                                      Ignored for heat and KS                                                            */
+    SWEPT_OPT_INJECT_ABORT = 8,   /* fault injection for tests of the error path (value 1; waits for the handle's work): marks the
+                                     handle as if a bounded wait of a launch-free kernel had given up.  The next sweep's waiting
+                                     warps leave early, and the mark is reported as described under "Conventions"            */
     SWEPT_OPT_PACK = 6,           /* heat fp32 on the streaming band kernel: 2 = every warp slot advances TWO bands (half a domain
                                      apart) in lock step on packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: half the FP
                                      instructions, per-component IEEE rounding, so the result is bit-identical); 1 = one band
@@ -271,7 +278,8 @@ int swept_problem_info(int problem, int *radius, int *stages, int *ncomp);
 /* Fill *info (caller-owned). */
 int swept_get_info(swept_handle_t h, swept_info_t *info);
 
-/* 1 if tile_width is legal for this handle and the selected kernel, else 0 (reason in swept_last_error). */
+/* 1 if swept_run accepts tile_width on this handle -- for the kernel family it would run that width on: the selected one, or, for the
+ * tuned width, the family swept_tune chose (swept_info_t.tuned_kernel) -- else 0 (reason in swept_last_error). */
 int swept_tile_width_ok(swept_handle_t h, int tile_width);
 
 /* Measure the plain-ALU peak the swept kernels are bound by: a dependent-free FMA chain of the
@@ -290,6 +298,10 @@ int swept_measure_smem_peak(double *bytes_per_s, double *ms, void *cuda_stream);
  * (two 64-bit shuffles -> DADD -> DFMA); [4] a tier exchanged through shared memory with one block barrier, 256 threads.
  * They bound what any decomposition of a small grid can reach.  SYNCHRONISES. */
 int swept_measure_latencies(double *cycles, void *cuda_stream);
+
+/* Wait (on the host) for everything enqueued through this handle and report whether a bounded wait of a launch-free sweep gave up
+ * since the last report: SWEPT_ECUDA once (the fields those sweeps ran on are invalid; the handle is usable again), else SWEPT_OK. */
+int swept_check(swept_handle_t h);
 
 /* Free the workspace and the handle.  The caller must have synchronised every stream it used. */
 int swept_destroy(swept_handle_t h);

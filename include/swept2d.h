@@ -43,7 +43,8 @@ typedef struct {
     int64_t launches_total;
 } swept2d_info_t;
 
-/* nx, ny: powers of two >= 8 (periodic neighbours by `& (n-1)`); dx = dy; `p` may be NULL (f64, alpha = 1).
+/* nx, ny: powers of two >= 8 (periodic neighbours by `& (n-1)`), nx <= 2^20, ny <= 2^18 (rows of blocks go on
+ * blockIdx.y, which the device limits to 65535); dx = dy; `p` may be NULL (f64, alpha = 1).
  * Allocates nx*ny elements of workspace on the current device.  Errors: SWEPT_EINVAL, SWEPT_ENOMEM, SWEPT_ECUDA. */
 int swept2d_create(swept2d_handle_t *out, int64_t nx, int64_t ny, double dx, double dt, const swept2d_params_t *p);
 

@@ -18,7 +18,7 @@ from typing import Optional
 HEAT, KS, EULER = 0, 1, 2
 F32, F64 = 0, 1
 KERNEL_SMEM, KERNEL_WAVE = 0, 1
-OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN, OPT_PACK, OPT_NAIVE_SHARE = 0, 1, 2, 3, 4, 5, 6, 7
+OPT_KERNEL, OPT_NAIVE_GRAPH, OPT_BLOCKS_PER_SM, OPT_WARPS_PER_BLOCK, OPT_SWEPT_GRAPH, OPT_CHAIN, OPT_PACK, OPT_NAIVE_SHARE, OPT_INJECT_ABORT = 0, 1, 2, 3, 4, 5, 6, 7, 8
 PACK_AUTO, PACK_OFF, PACK_ON = 0, 1, 2
 LAUNCH_CLASSIC, LAUNCH_UP, LAUNCH_DIAMOND, LAUNCH_DOWN, LAUNCH_CHAIN, LAUNCH_BAND, LAUNCH_RING = 0, 1, 2, 3, 4, 5, 6
 LAUNCH_NAMES = {0: "classic", 1: "up", 2: "diamond", 3: "down", 4: "chain", 5: "band", 6: "ring"}
@@ -33,7 +33,7 @@ SYMBOLS = (
     "swept_create", "swept_run", "naive_run", "swept_tune", "swept_run_host", "swept_set_option", "swept_get_info",
     "swept_tile_width_ok", "swept_measure_alu_peak", "swept_destroy", "swept_last_error", "swept_version", "swept_plan",
     "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak", "swept_measure_latencies",
-    "swept_run_static",
+    "swept_run_static", "swept_check",
     # include/swept2d.h
     "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy",
 )
@@ -111,6 +111,7 @@ def lib() -> ctypes.CDLL:
     L.swept_tile_width_ok.argtypes = [vp, ci]
     L.swept_measure_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
     L.swept_destroy.argtypes = [vp]
+    L.swept_check.argtypes = [vp]
     L.swept_plan.argtypes = [ci, ci, i64, i64, ci, ci, ci, ctypes.POINTER(_Launch), i64]
     L.swept_band_layout.argtypes = [ci, ci, ci, ctypes.POINTER(_BandLayout)]
     L.swept_band_owner.argtypes = [ctypes.POINTER(_BandLayout), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
@@ -218,6 +219,10 @@ class Solver:
 
     def set_option(self, key: int, value: int) -> None:
         _check(lib().swept_set_option(self._h, int(key), int(value)))
+
+    def check(self) -> None:
+        """swept_check: wait for the handle's work; raises SweptError(ECUDA) once if a launch-free sweep gave up a bounded wait."""
+        _check(lib().swept_check(self._h))
 
     def tile_width_ok(self, tile_width: int) -> bool:
         return bool(lib().swept_tile_width_ok(self._h, int(tile_width)))

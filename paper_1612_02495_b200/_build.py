@@ -20,7 +20,10 @@ HEADERS = ["internal.h", "stencils.cuh", "swept_wave.cuh", "swept_band.cuh", "sw
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-fmad=false",
     "-Xcompiler", "-fPIC,-ffp-contract=off",
-] + os.environ.get("SWEPT_NVCC_EXTRA", "").split()
+]
+# The flags are fixed: no environment variable reaches the compiler, so a product build cannot be steered into another kernel.
+# Objects built with other flags (an older checkout, a hand-run nvcc) are rebuilt: the flags are stamped beside them.
+STAMP = os.path.join(OBJ, "flags.stamp")
 
 
 def _nvcc() -> str:
@@ -41,6 +44,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     hdrs = [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS] + [os.path.abspath(__file__)]
     nvcc = _nvcc()
+    stamp = " ".join([nvcc, *NVCC_FLAGS])
+    if not os.path.exists(STAMP) or open(STAMP).read() != stamp:
+        force = True
     jobs = []
     objs = []
     for src in SOURCES:
@@ -62,6 +68,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             list(ex.map(run, jobs))
     if force or jobs or _stale(OUT, objs):
         run([nvcc, "-shared", "-o", OUT, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    with open(STAMP, "w") as f:
+        f.write(stamp)
     return OUT
 
 

@@ -213,9 +213,11 @@ static int check_width(const swept_ctx *h, int W, int kernel, bool set_err) {
     return 1;
 }
 
+static int tuned_family(const swept_ctx *h, int W);
+
 extern "C" int swept_tile_width_ok(swept_handle_t h, int tile_width) {
     if (!h) { fail(SWEPT_EINVAL, "swept_tile_width_ok: NULL handle"); return 0; }
-    return check_width(h, tile_width, h->kernel, true);
+    return check_width(h, tile_width, tuned_family(h, tile_width), true);    // the family swept_run would run this width on
 }
 
 // The kernel family swept_run uses for width W: the option's, except that under the default options (register kernels, launch-free
@@ -245,18 +247,22 @@ static int default_width(const swept_ctx *h, int *kernel) {
 // ---- entry / exit of every call that enqueues work on a handle ---------------------------------------------------
 // The handle's device (the kernels' shared-memory opt-ins and the scratch are per device) must be current; a wait that gave up
 // in an earlier launch-free sweep is reported once; the stream first waits for the handle's previous call (any stream).
+// A bounded wait gave up (the pinned copy of the abort word is set): wait for everything the handle enqueued, clear the word on
+// both sides so that the handle is usable again, and report once.
+static int report_abort(swept_ctx *h, const char *who) {
+    cudaEventSynchronize(h->busy);
+    *h->abort_seen = 0;
+    cudaMemset(h->sync_base, 0, SYNC_HEADER);
+    return fail(SWEPT_ECUDA, "%s: an earlier launch-free sweep on this handle gave up waiting for a tile that never completed "
+                             "(was the handle used from two host threads at once?); the field it ran on is invalid", who);
+}
+
 static int handle_enter(swept_ctx *h, cudaStream_t st, const char *who) {
     int dev = -1;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return fail_cuda(e, who);
     if (dev != h->device) return fail(SWEPT_EINVAL, "%s: the handle was created on device %d but device %d is current", who, h->device, dev);
-    if (*(volatile unsigned *)h->abort_seen) {
-        cudaStreamSynchronize(st);
-        *h->abort_seen = 0;
-        cudaMemset(h->sync_base, 0, SYNC_HEADER);
-        return fail(SWEPT_ECUDA, "%s: an earlier launch-free sweep on this handle gave up waiting for a tile that never completed "
-                                 "(was the handle used from two host threads at once?); the field it ran on is invalid", who);
-    }
+    if (*(volatile unsigned *)h->abort_seen) return report_abort(h, who);
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
     if (cs == cudaStreamCaptureStatusNone) {
@@ -272,6 +278,14 @@ static void handle_leave(swept_ctx *h, cudaStream_t st) {
     cudaMemcpyAsync(h->abort_seen, h->sync_base, sizeof(unsigned), cudaMemcpyDeviceToHost, st);
     cudaEventRecord(h->busy, st);
 }
+
+// Every exit path of a call that passed handle_enter records the busy event, also the error returns: work that was enqueued before
+// the error is then still ahead of whatever the next call (on any stream) enqueues.
+struct LeaveGuard {
+    swept_ctx *h;
+    cudaStream_t st;
+    ~LeaveGuard() { handle_leave(h, st); }
+};
 
 // ---- classic path (row A2) -----------------------------------------------------------------------------------
 // Enqueue nsteps classic timesteps.  Heat ping-pongs u and work (and copies back after an odd count); two-stage
@@ -341,6 +355,7 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = handle_enter(h, st, "naive_run"))) return rc;
+    LeaveGuard leave{h, st};
     int64_t launches = 0;
     if (h->naive_graph && nsteps >= 2) {
         // a graph of `chunk` timesteps (even, so heat's ping-pong ends in d_u), replayed; the rest as plain launches
@@ -361,7 +376,6 @@ extern "C" int naive_run(swept_handle_t h, void *d_u, int64_t nsteps, void *cuda
         cudaError_t e = enqueue_classic(h, d_u, nsteps, st, &launches);
         if (e != cudaSuccess) return fail_cuda(e, "naive_run");
     }
-    handle_leave(h, st);
     h->launches_last = launches;
     h->launches_total += launches;
     return SWEPT_OK;
@@ -518,6 +532,7 @@ extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_w
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = handle_enter(h, st, "swept_run"))) return rc;
+    LeaveGuard leave{h, st};
     int64_t launches = 0;
     if (h->swept_graph && nsteps > 0) {
         const int chain = effective_chain(h, W), cap = effective_cap(h, W);
@@ -532,7 +547,6 @@ extern "C" int swept_run(swept_handle_t h, void *d_u, int64_t nsteps, int tile_w
         cudaError_t e = enqueue_swept(h, kernel, d_u, nsteps, W, st, &launches);
         if (e != cudaSuccess) return fail_cuda(e, "swept_run");
     }
-    handle_leave(h, st);
     h->launches_last = launches;
     h->launches_total += launches;
     return SWEPT_OK;
@@ -545,6 +559,7 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     if (blocks_per_sm_cap < 0) return fail(SWEPT_EINVAL, "swept_tune: blocks_per_sm_cap < 0");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = handle_enter(h, st, "swept_tune"))) return rc;
+    LeaveGuard leave{h, st};
     const int saved_cap = h->blocks_per_sm, saved_graph = h->swept_graph;
     h->blocks_per_sm = blocks_per_sm_cap;
     h->swept_graph = 0;
@@ -635,7 +650,6 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
     cudaEventDestroy(e1);
     h->blocks_per_sm = saved_cap;
     h->swept_graph = saved_graph;
-    handle_leave(h, st);
     if (e != cudaSuccess) return fail_cuda(e, "swept_tune");
     drop_graphs(h);                                      // a cached swept graph was captured with the pre-tune launch shape
     h->tuned_tile_width = best;
@@ -656,6 +670,7 @@ extern "C" int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int t
     cudaError_t e;
     int rc0 = handle_enter(h, st, "swept_run_host");
     if (rc0) return rc0;
+    LeaveGuard leave{h, st};
     if (!h->host_stage) {
         e = cudaMalloc(&h->host_stage, h->field_bytes);
         if (e != cudaSuccess) { cudaGetLastError(); h->host_stage = nullptr; return fail(SWEPT_ENOMEM, "swept_run_host: cudaMalloc: %s", cudaGetErrorString(e)); }
@@ -668,6 +683,19 @@ extern "C" int swept_run_host(swept_handle_t h, void *h_u, int64_t nsteps, int t
     if (e != cudaSuccess) return fail_cuda(e, "swept_run_host: D2H");
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return fail_cuda(e, "swept_run_host: synchronize");
+    if (*(volatile unsigned *)h->abort_seen) return report_abort(h, "swept_run_host");    // h_u holds garbage: say so now
+    return SWEPT_OK;
+}
+
+extern "C" int swept_check(swept_handle_t h) {
+    if (!h) return fail(SWEPT_EINVAL, "swept_check: NULL handle");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(e, "swept_check");
+    if (dev != h->device) return fail(SWEPT_EINVAL, "swept_check: the handle was created on device %d but device %d is current", h->device, dev);
+    e = cudaEventSynchronize(h->busy);       // behind the last call's kernels and the copy of the abort word
+    if (e != cudaSuccess) return fail_cuda(e, "swept_check");
+    if (*(volatile unsigned *)h->abort_seen) return report_abort(h, "swept_check");
     return SWEPT_OK;
 }
 
@@ -701,6 +729,14 @@ extern "C" int swept_set_option(swept_handle_t h, int key, int value) {
             h->pack = value;
             drop_graphs(h);
             return SWEPT_OK;
+        case SWEPT_OPT_INJECT_ABORT: {
+            if (value != 1) return fail(SWEPT_EINVAL, "swept_set_option: INJECT_ABORT takes 1");
+            const unsigned one = 1;
+            cudaError_t e = cudaEventSynchronize(h->busy);
+            if (e == cudaSuccess) e = cudaMemcpy(h->sync_base, &one, sizeof one, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) return fail_cuda(e, "swept_set_option(INJECT_ABORT)");
+            return SWEPT_OK;
+        }
         case SWEPT_OPT_BLOCKS_PER_SM:
             if (value < 0 || value > 32) return fail(SWEPT_EINVAL, "swept_set_option: BLOCKS_PER_SM takes 0..32");
             h->blocks_per_sm = value;

@@ -252,13 +252,7 @@ __device__ __forceinline__ void tier32f(T (&a0)[16][2], T (&a1)[16][2], const in
     T(&src)[16][2] = SRC0 ? a0 : a1;
     T(&dst)[16][2] = SRC0 ? a1 : a0;
     // register rows per uniform branch (measured, 8192^2, GPts*steps/s: fp64 1: 345, 2: 414, 4: 425; fp32 2: 756, 4: 813, 8: 785, 16: 640)
-#ifndef H2D_RG64
-#define H2D_RG64 4
-#endif
-#ifndef H2D_RG32
-#define H2D_RG32 4
-#endif
-    constexpr int RG = sizeof(T) == 4 ? H2D_RG32 : H2D_RG64;
+    constexpr int RG = 4;
     const unsigned rows = 0xffffu & ~((1u << ya) - 1u);    // register rows ya .. 15 (warp-uniform)
     const int x0 = 2 * l;
     const unsigned mine0 = (x0 >= xa && x0 < xb) ? rows : 0u, mine1 = (x0 + 1 >= xa && x0 + 1 < xb) ? rows : 0u;
@@ -463,8 +457,9 @@ extern "C" int swept2d_create(swept2d_handle_t *out, int64_t nx, int64_t ny, dou
     const int dtype = p ? p->dtype : SWEPT_F64;
     const double alpha = p ? p->alpha : 1.0;
     if (dtype != SWEPT_F32 && dtype != SWEPT_F64) return swept_fail(SWEPT_EINVAL, "swept2d_create: unknown dtype %d", dtype);
-    if (!pow2(nx) || !pow2(ny) || nx < 8 || ny < 8 || nx > ((int64_t)1 << 20) || ny > ((int64_t)1 << 20))
-        return swept_fail(SWEPT_EINVAL, "swept2d_create: nx=%lld, ny=%lld must be powers of two in [8, 2^20]", (long long)nx, (long long)ny);
+    // ny / 8 rows of blocks must fit gridDim.y (65535): the classic kernel and the narrowest shared-memory tiles put rows on blockIdx.y
+    if (!pow2(nx) || !pow2(ny) || nx < 8 || ny < 8 || nx > ((int64_t)1 << 20) || ny > ((int64_t)1 << 18))
+        return swept_fail(SWEPT_EINVAL, "swept2d_create: nx=%lld, ny=%lld must be powers of two, nx in [8, 2^20], ny in [8, 2^18]", (long long)nx, (long long)ny);
     if (!isfinite(dx) || !isfinite(dt) || dx <= 0.0 || dt <= 0.0 || !(isfinite(alpha) && alpha > 0.0))
         return swept_fail(SWEPT_EINVAL, "swept2d_create: dx, dt and alpha must be finite and positive");
     int dev = 0;

@@ -58,11 +58,6 @@ template <> __device__ __forceinline__ float2p shfl_up1<float2p>(float2p v) {
     return float2p(__shfl_up_sync(0xffffffffu, v.x, 1), __shfl_up_sync(0xffffffffu, v.y, 1));
 }
 
-#ifndef STEADY_UNROLL
-#define STEADY_UNROLL 1
-#endif
-constexpr int STEADY_UNROLL_N = STEADY_UNROLL;      // iterations of the steady loop unrolled together
-
 template <class P, int PW> struct BandGeom {
     using T = typename P::real;
     static constexpr int H = P::H, NC = P::NC, D = 2 * H, SR = band_sr<P, PW>();
@@ -120,10 +115,7 @@ __device__ __forceinline__ void band_super_rows(typename P::real (&X)[P::NC][2 *
     using T = typename P::real;
     constexpr int H = P::H, NC = P::NC, D = 2 * H, NP = PW / D;
     T old[SR][D][NC];
-#ifndef BAND_HEAT_BREADTH_FIRST
-#define BAND_HEAT_BREADTH_FIRST 1
-#endif
-    if constexpr (BAND_HEAT_BREADTH_FIRST && !P::GROUPED && H == 1 && NC == 1 && P::S == 1) {
+    if constexpr (!P::GROUPED && H == 1 && NC == 1 && P::S == 1) {
         // Heat: the SR x D point updates of one step are independent (super-row s + 1 runs one point behind super-row s): all sums,
         // then all products, then all fused multiply-adds, in that source order, so that a warp alone on its scheduler keeps SR D
         // chains in flight instead of the two or three the point-by-point order left it (ncu, nx = 2^18: `wait` 1.25 per issue)
@@ -381,7 +373,8 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                         if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
                     }
                 }
-                if (__any_sync(0xffffffffu, dead)) return;    // (also the warp barrier behind lane 0's acquire)
+                __syncwarp();                                     // orders the other lanes' loads behind the polling lanes' acquire
+                if (__any_sync(0xffffffffu, dead)) return;
                 const int64_t g0 = g0_of(bandf, pf);
 #pragma unroll
                 for (int sr = 0; sr < SR; ++sr) {
@@ -416,7 +409,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                 int J = (K0 - lane) & (NJI - 1);
                 const T *fp = feed;
                 T *op = outr + ((K0 - 31) & 63) * SR * D;     // lane 31's slot of local time K0 - 31
-#pragma unroll(STEADY_UNROLL_N)
+#pragma unroll 1
                 for (int it = 0; it < 32; ++it) {
                     T recv[SR][NC][D];
 #pragma unroll
@@ -527,6 +520,7 @@ __global__ void __launch_bounds__((band_max_threads<P, PW, TIGHT>())) swept_band
                 if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
             }
         }
+        __syncwarp();                                     // orders the other lanes' loads behind the polling lanes' acquire
         if (__any_sync(0xffffffffu, dead)) return;
     }
     // ---- all phases done: column i of a band ended at x = g0(band, q) + i - H rt; registers hold band k-1's flat values, the

@@ -41,22 +41,15 @@ namespace swept {
 
 template <class P, int PW> struct RingGeom {
     using T = typename P::real;
-#ifndef RING_EXP_SR
-#define RING_EXP_SR 0
-#endif
-#ifndef RING_EXP_CH8
-#define RING_EXP_CH8 0
-#endif
     static constexpr int H = P::H, NC = P::NC, D = 2 * H;
     static constexpr int W = 32 * PW, NJ = W / D, NP = PW / D, L = W / D, CTR = W / 2;
-    static constexpr int SR0 = band_sr<P, PW>();
-    static constexpr int SR = (RING_EXP_SR && H == 1 && NJ / SR0 == 64 && SR0 > 1) ? SR0 / 2 : SR0;
+    static constexpr int SR = band_sr<P, PW>();
     static constexpr int NJI = NJ / SR;                       // iterations per tile
     // Iterations per chunk and ring capacity.  Heat iterations are short (60..150 cycles for a warp alone on its scheduler), so the
     // rings must cover a few thousand cycles of exchange latency: chunks of 16 (32 for the long tiles), four (two) chunks of ring.
     // KS / Euler iterations cost hundreds to thousands of cycles and their rows are wide (D = 4, Euler 3 fields): chunks of 8 (16)
     // and two chunks of ring keep the rings at 1..3 KB per warp, which is what lets the parked bands of the largest grids fit.
-    static constexpr int CH = H == 1 ? (NJI >= 128 ? 32 : (RING_EXP_CH8 ? 8 : 16)) : (NJI >= 128 ? 16 : 8);
+    static constexpr int CH = H == 1 ? (NJI >= 128 ? 32 : 16) : (NJI >= 128 ? 16 : 8);
     static constexpr int NCH = NJI / CH;                      // chunks per tile
     static constexpr int CAP = (H == 1 && CH == 16 ? 4 : 2) * CH;   // feed ring capacity in iterations (prefetch depth CAP - CH)
     static constexpr int LAGC = (31 + CH) / CH;               // chunks between the end of a chunk and the boundary at which lane 31 is through it
@@ -82,9 +75,6 @@ constexpr int RING_ROOMY = 3;
 template <class P, int PW> constexpr int ring_nwmax() {
     const int est = P::NC * (2 * P::H + PW) * (int)(sizeof(typename P::real) / 4) + (P::GROUPED ? 110 : 56 + 16 * (P::H - 1));
     int warps = 65536 / (32 * est);
-#ifdef RING_EXP_EULER_NW
-    if (P::GROUPED && sizeof(typename P::real) == 8 && PW == 8) warps = RING_EXP_EULER_NW;
-#endif
     if (P::H == 2 && !P::GROUPED && sizeof(typename P::real) == 8 && PW == 32) warps = 8;   // KS fp64, 32 points per lane: spills below ~200 registers
     warps = warps >= 4 ? (warps & ~3) : 4;
     return (warps > 28 ? 28 : warps) - 1;
@@ -373,20 +363,14 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
             }
         }
         __syncwarp();
-#ifdef RING_EXP_NOREL
-        if (lane == 0) *reinterpret_cast<volatile unsigned *>(&my->k0) = (unsigned)K0;
-#else
         if (lane == 0) st_release_cta_shared(&my->k0, (unsigned)K0);
-#endif
         {
             const int need_feed = K0 < lt_end ? (K0 + CH < lt_end ? K0 + CH : lt_end) : 0;
             SpinWatch polls;
             bool dead = false;
-#ifndef RING_EXP_NOWAIT                                   // (experiment: the rate with a free exchange -- results are wrong)
             while ((int)ld_acquire_cta_shared(&my->feed) < need_feed) {
                 if (spin_gives_up(polls, abort_word_of(prog))) { dead = true; break; }
             }
-#endif
             if (__any_sync(0xffffffffu, dead)) return;
         }
 
@@ -404,7 +388,7 @@ __global__ void __launch_bounds__(32 * (NWMAX + 1)) swept_ring_kernel(typename P
                 constexpr bool SWAP = decltype(swap_tag)::value;
                 int J = (K0 - lane) & (NJI - 1);
                 int fs = K0 & (CAP - 1), os = (K0 - 31) & (OCAP - 1);     // ring slots: lane 0's local time K0, lane 31's K0 - 31
-#pragma unroll(STEADY_UNROLL_N)
+#pragma unroll 1
                 for (int it = 0; it < CH; ++it) {
                     const T *fp = feed + fs * SR * D;
                     T recv[SR][NC][D];

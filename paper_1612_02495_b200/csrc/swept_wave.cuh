@@ -292,7 +292,8 @@ __global__ void __launch_bounds__((chain_max_threads<P, PW>()), (chain_min_block
                     if (spin_gives_up(polls, abort_word_of(counter))) { dead = true; break; }
                 }
             }
-            if (__any_sync(0xffffffffu, dead)) return;        // (also the warp barrier that orders the other lanes behind the acquire)
+            __syncwarp();                                     // orders the other lanes' loads behind the polling lanes' acquire
+            if (__any_sync(0xffffffffu, dead)) return;
         }
         const int64_t g0 = (int64_t)t * W + ((p & 1) ? W / 2 : 0);
         if (p == 0) wave_tile<P, PW, MODE_UP, true>(u, w, nx, g0, io, c, lane);
@@ -347,6 +348,7 @@ __global__ void __launch_bounds__(256) swept_chain_ins_kernel(typename P::real *
                     }
                 }
             }
+            __syncwarp();                                     // orders the other lanes' loads behind the polling lanes' acquire
             if (__any_sync(0xffffffffu, dead)) return;
         }
         const int64_t g0 = odd ? (int64_t)t * W - W / 2 : (int64_t)t * W;

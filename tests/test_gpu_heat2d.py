@@ -101,6 +101,19 @@ def test_illegal_arguments_2d():
             s.set_option(sw.OPT2D_KERNEL, 7)
 
 
+def test_skinny_2d_grid_at_the_row_limit():
+    """ny = 2^18 is the tallest grid the header allows (ny / 8 rows of blocks on blockIdx.y): every path launches and agrees;
+    one row more is refused at creation instead of failing at launch."""
+    nx, ny = 8, 1 << 18
+    u0 = wl.heat2d_field(nx, ny)
+    want, _ = _run(nx, ny, np.float64, 5, None, u0=u0)
+    assert np.isfinite(want).all()
+    got, _ = _run(nx, ny, np.float64, 5, 8, u0=u0)                # one classic remainder step, then one half-cycle of W = 8 (4 timesteps)
+    assert_bits_equal(got, want, "swept W = 8 on 8 x 2^18")
+    with pytest.raises(sw.SweptError):
+        sw.Solver2D(8, 1 << 19, 1.0, 0.1)
+
+
 def test_the_two_2d_kernels_agree():
     """The register kernel and the shared-memory kernel run the same regions in the same tier order with the same store rule:
     identical fields after 1, 2 and 3 half-cycles (odd and even closing alignment)."""

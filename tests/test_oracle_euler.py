@@ -242,6 +242,35 @@ def test_minmod_limiter_is_tvd_on_a_square_contact():
     _check_tvd_contact(_oracle_euler)
 
 
+def _check_rusanov_speed(euler):
+    """Which side's signal speed the Rusanov dissipation takes.  Semi-discrete limit: for dt -> 0 the predictor state tends to U^m, so
+    one step changes cell i by -lambda (F_{i+1/2}(U^m) - F_{i-1/2}(U^m)) + O(lambda^2).  Datum: two constant states at rest on 8 cells
+    (every minmod slope is zero: a cell next to the jump has one zero difference), gamma = 2 so that c^2 = 2 p / rho is 1 on one side
+    and 4 on the other: |u| + c = 1 and 2 exactly, a = max = 2.  At the jump face f = (0, p, 0) on both sides, so by the definition
+    of the flux, F = (f_L + f_R)/2 - (a/2)(U_R - U_L) = (-(a/2) [rho], (p_L + p_R)/2, -(a/2) [E]) with E = p / (gamma - 1) = p; the
+    faces inside a state carry (0, p, 0).  Expected change of the cells beside the jump, in units of lambda, with a = 2:
+    rho +-1, m -+(9/4 - p_own), E +-7/2.  With a = min = 1 the density and energy changes halve.  Both orientations of the jump are on
+    the periodic grid (faces 3|4 and 7|0), so taking one fixed side's speed fails as well."""
+    gamma, lam = 2.0, 1e-6
+    rho = np.array([1.0] * 4 + [2.0] * 4)
+    p = np.array([0.5] * 4 + [4.0] * 4)                      # c = sqrt(2 p / rho) = 1 | 2
+    U0 = np.stack([rho, np.zeros(8), p / (gamma - 1.0)])
+    U1 = euler(U0, 1, gamma, 1.0, lam)
+    d = (U1 - U0) / lam
+    a = 2.0
+    drho, dE, pm = 0.5 * a * (2.0 - 1.0), 0.5 * a * (4.0 - 0.5), 0.5 * (0.5 + 4.0)
+    want = np.zeros((3, 8))
+    #            cell 0 (face 7|0)   cell 3 (face 3|4)   cell 4 (face 3|4)   cell 7 (face 7|0)
+    want[0, [0, 3, 4, 7]] = [+drho, +drho, -drho, -drho]
+    want[1, [0, 3, 4, 7]] = [-(0.5 - pm), -(pm - 0.5), -(4.0 - pm), -(pm - 4.0)]
+    want[2, [0, 3, 4, 7]] = [+dE, +dE, -dE, -dE]
+    assert np.max(np.abs(d - want)) < 1e-4, (d, want)
+
+
+def test_rusanov_takes_the_larger_signal_speed():
+    _check_rusanov_speed(_oracle_euler)
+
+
 # name -> (text in oracle/schemes.inc, replacement, the pin that must catch it)
 MUTANTS = {
     "first-order (sigma = 0)": ("if (p > (REAL)0.0) return (R_FABS(a) < R_FABS(b)) ? a : b;", "if (p > (REAL)0.0) return (REAL)0.0;", "order"),
@@ -251,7 +280,11 @@ MUTANTS = {
     "full-step predictor (lambda for lambda/2)": ("FN(euler_stage)(U, U, Us, nx, lamh, gamma, gm1)", "FN(euler_stage)(U, U, Us, nx, lam, gamma, gm1)", "order"),
     "forward Euler (corrector from U^m)": ("FN(euler_stage)(Us, U, Un, nx, lam, gamma, gm1)", "FN(euler_stage)(U, U, Un, nx, lam, gamma, gm1)", "order"),
     "face states of the wrong sign": ("R_FMA((REAL)-0.5, sp, w[ip])", "R_FMA((REAL)0.5, sp, w[ip])", "order"),
+    "Rusanov speed: the smaller side": ("const REAL a = R_FMAX(sL, sR);", "const REAL a = (sL < sR) ? sL : sR;", "speed"),
+    "Rusanov speed: the left side only": ("const REAL a = R_FMAX(sL, sR);", "const REAL a = sL;", "speed"),
+    "Rusanov speed: the mean of the sides": ("const REAL a = R_FMAX(sL, sR);", "const REAL a = (REAL)0.5 * (sL + sR);", "speed"),
 }
+PINS = {"order": lambda f: _check_second_order(f), "tvd": lambda f: _check_tvd_contact(f), "speed": lambda f: _check_rusanov_speed(f)}
 
 
 @pytest.mark.parametrize("name", list(MUTANTS))
@@ -282,4 +315,4 @@ def test_mutants_of_the_oracle_fail_the_second_order_pins(name, tmp_path):
         return a
 
     with pytest.raises(AssertionError):
-        (_check_second_order if pin == "order" else _check_tvd_contact)(mutant)
+        PINS[pin](mutant)

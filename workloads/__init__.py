@@ -92,20 +92,21 @@ def heat_config2(nx: int, seed: int = SEED_MODES) -> Workload:
     return Workload(HEAT, nx, dx, dt, u0[None, :], nsteps=50_000, name="heat-config2")
 
 
-def heat_noise(nx: int, seed: int = SEED_NOISE) -> Workload:
-    """Grid-scale U[-1,1] noise: every step changes every value at O(1) (SURVEY §8(c) 'sensitive')."""
-    dx, dt = heat_grid(nx)
+def heat_noise(nx: int, seed: int = SEED_NOISE, r: float = 0.25, alpha: float = 1.0) -> Workload:
+    """Grid-scale U[-1,1] noise: every step changes every value at O(1) (SURVEY §8(c) 'sensitive').  r = alpha dt / dx^2: with the
+    configs' r = 1/4 every product of the update is exact in binary; any other r (and alpha != 1) makes rounding order matter."""
+    dx, dt = heat_grid(nx, r, alpha)
     u0 = np.random.default_rng(seed).uniform(-1.0, 1.0, nx)
-    return Workload(HEAT, nx, dx, dt, u0[None, :], name="heat-noise")
+    return Workload(HEAT, nx, dx, dt, u0[None, :], alpha=alpha, name="heat-noise")
 
 
-def heat_rod(nx: int, seed: int = SEED_NOISE) -> Workload:
+def heat_rod(nx: int, seed: int = SEED_NOISE, r: float = 0.25, alpha: float = 1.0) -> Workload:
     """The paper's heat problem: a rod with an initial temperature gradient and insulated ends -- a linear ramp
     3 -> 0 from the left end to the right end plus grid-scale U[-1,1] noise, so that every step changes every value and the
     two ends differ (a periodic ring would leak across the seam).  Used with boundary = insulated."""
-    dx, dt = heat_grid(nx)
+    dx, dt = heat_grid(nx, r, alpha)
     u0 = 3.0 * (1.0 - (np.arange(nx) + 0.5) / nx) + np.random.default_rng(seed).uniform(-1.0, 1.0, nx)
-    return Workload(HEAT, nx, dx, dt, u0[None, :], name="heat-rod")
+    return Workload(HEAT, nx, dx, dt, u0[None, :], alpha=alpha, name="heat-rod")
 
 
 # ----------------------------------------------------------------------------------------------
