@@ -96,6 +96,7 @@ def parse():
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="SWEPT_OPT_BLOCKS_PER_SM for the per-tile kernels (0 = none / tuned)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-classic", action="store_true", help="skip the classic-path context run (profiling)")
+    ap.add_argument("--no-range", action="store_true", help="skip the `sweep` points at nx = 2^11, 2^14, 2^17, 2^20 (profiling)")
     ap.add_argument("--probe", action="store_true", help="print the library's microbenchmarks as one JSON line: FP64 / FP32 FMA-chain peaks, shared-memory read peak, "
                     "latency probes (swept_measure_latencies): the denominators and bounds DESIGN.md quotes")
     ap.add_argument("--heat2d", action="store_true", help="secondary measurement (SURVEY.md section 8(f) NEXT-4): the 2-D swept rule against the classic "
@@ -257,6 +258,53 @@ def run_reference(args):
 # range, every legal tile width against the classic path, best width kept.
 # ---------------------------------------------------------------------------------------------------------------
 SWEEP_NX = {"heat": range(11, 23), "ks": range(14, 21), "euler": range(12, 21)}
+
+
+def metric_range(args, sizes=(11, 14, 17, 20)):
+    """BASELINE.json's metric is quoted over nx = 2^11 ... 2^22 (the paper's experiment is the sweep, not one
+    size).  The headline line times the largest size; this adds four more points of the same problem / dtype at the config's full
+    step count -- the default swept path (swept_tune's choice, as in the headline) and the graph-launched classic path -- so that
+    the driver's own run witnesses the range.  Each point: one warm-up call, then the median of 3 calls, CUDA events on the
+    launching stream, L2 flushed between calls."""
+    import torch
+
+    import paper_1612_02495_b200 as sw
+
+    np_dtype = np.float64 if args.dtype == "f64" else np.float32
+    sw_dtype = sw.F64 if args.dtype == "f64" else sw.F32
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn):
+        fn()
+        ts = []
+        for _ in range(3):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream); e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        return statistics.median(ts)
+
+    points = []
+    for lg in sizes:
+        nx = 1 << lg
+        w = wl.make(args.problem, nx, "config")
+        u0 = torch.from_numpy(w.initial(np_dtype)).cuda()
+        u = u0.clone()
+        with sw.Solver(w.problem, nx, w.dx, w.dt, dtype=sw_dtype, alpha=w.alpha, gamma=w.gamma) as s:
+            W = s.tune(u.clone())
+            t_swept = timed(lambda: s.swept_run(u, w.nsteps, W))
+            info = s.info()
+            kname = "smem" if info["tuned_kernel"] == sw.KERNEL_SMEM else sw.LAUNCH_NAMES.get(info["last_sweep_launch"], "?")
+            launches = info["launches_last_call"]
+            s.set_option(sw.OPT_NAIVE_GRAPH, 1)
+            u.copy_(u0)
+            t_classic = timed(lambda: s.naive_run(u, w.nsteps))
+        points.append({"log2_nx": lg, "nsteps": w.nsteps, "swept": nx * w.nsteps / t_swept / 1e9, "tile_width": W, "kernel": kname,
+                       "launches_per_run": int(launches), "classic_graph": nx * w.nsteps / t_classic / 1e9,
+                       "speedup": t_classic / t_swept})
+    return {"unit": "GPts*steps/s", "what": f"{args.problem} {args.dtype}, config step count, tuned swept path vs graph-launched classic path; "
+                                            "median of 3 calls after a warm-up call, L2 flushed between calls", "points": points}
 
 
 def run_sweep(args):
@@ -708,6 +756,10 @@ def main():
         cpu = {"value": rate / 1e9, "unit": "GPts*steps/s", "cores": cores, "kind": "oracle", "value_1_thread": rate1 / 1e9,
                "sample": f"{n} of {w.nsteps} timesteps at nx={w.nx} ({el:.1f} s)"}
 
+    sweep = None
+    if rank == 0 and world == 1 and not (args.no_range or args.no_classic) and args.boundary == "periodic":
+        sweep = metric_range(args)
+
     out = {
         "metric": "grid-point updates/sec", "value": value, "unit": "GPts*steps/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": t_dev_max / args.steps * 1e3, "higher_is_better": True,
@@ -727,6 +779,7 @@ def main():
         "roofline": roofline,
         "cpu_baseline": cpu,
         "classic": classic,
+        "sweep": sweep,
     }
     print(json.dumps(out))
     if world > 1:
