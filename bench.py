@@ -510,16 +510,55 @@ def run_heat2d(args):
             u.copy_(u0)
             t = timed(lambda: s.swept_run(u, nsteps, W))
             res[f"swept W={W} ({kname})"] = n * n * nsteps / t / 1e9
+        # e2e: the same run through swept2d_run_host -- H2D of the field from pinned host memory, the default swept path (register
+        # kernel, W = 32), D2H of the result, synchronise -- wall-clock around the C-ABI call, median of 3
+        s.set_option(sw.OPT2D_KERNEL, sw.KERNEL2D_WARP)
+        h_u = u0.cpu().pin_memory()
+        s.run_host(h_u, nsteps, 32)
+        ts = []
+        for _ in range(3):
+            h_u.copy_(u0)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            s.run_host(h_u, nsteps, 32)
+            ts.append(time.perf_counter() - t0)
+        e2e_val = n * n * nsteps / statistics.median(ts) / 1e9
     try:
         hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_src = "measured (MEASURED_PEAKS.json)"
     except Exception:
-        hbm_peak = 6650.0
+        hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
     es = u.element_size()
     best = max((k for k in res if k.startswith("swept")), key=res.get)
+    Wb = int(best.split("W=")[1].split()[0])
+    # roofline of the swept path: by algorithmic bytes it would be HBM-bound (7 values per point per half-cycle of W/2 timesteps, see
+    # below), by arithmetic FP-pipe-bound (5 FP instructions per update: 3 adds, 1 multiply, 1 fma); it reaches neither (DESIGN.md
+    # section 5.8: issue- and latency-bound at 8 warps per SM), so both fractions are stated and `bound` names the nearer one
+    bytes_per_update = 7 * es / (Wb // 2)
+    hbm_frac = res[best] * bytes_per_update / hbm_peak
+    alu_peak = 148 * (64 if args.dtype == "f64" else 128) * 1.965e-3          # T thread-level FP instr/s, nominal pipe
+    alu_frac = res[best] * 5e-3 / alu_peak
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        a0 = wl.heat2d_field(n, n).astype(np_dtype)
+        oracle.heat2d(a0, 1, 1.0, dx, dt)
+        t0 = time.perf_counter(); oracle.heat2d(a0, 4, 1.0, dx, dt); t4 = time.perf_counter() - t0
+        k = int(max(4, min(nsteps, 12.0 / max(t4 / 4, 1e-9))))
+        t0 = time.perf_counter(); oracle.heat2d(a0, k, 1.0, dx, dt); el = time.perf_counter() - t0
+        cpu = {"value": n * n * k / el / 1e9, "unit": "GPts*steps/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{k} of {nsteps} timesteps at {n} x {n} ({el:.1f} s)"}
     print(json.dumps({
         "metric": "grid-point updates/sec (2-D heat, secondary)", "unit": "GPts*steps/s", "value": res[best], "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": f"2-D heat FTCS 5-point, periodic {n} x {n}, Fo = 0.2, {nsteps} timesteps; field {n * n * es >> 20} MiB (larger than L2)", "best": best},
         "results": res, "speedup_swept_over_classic": res[best] / res["classic"],
+        "e2e": {"value": e2e_val, "unit": "GPts*steps/s", "h2d_bytes_per_step": n * n * es, "d2h_bytes_per_step": n * n * es,
+                "what": "swept2d_run_host, register kernel W = 32, pinned host buffer, wall clock around the call, median of 3"},
+        "roofline": {"bound": "hbm" if hbm_frac >= alu_frac else "alu", "kernel": best, "achieved": res[best] * bytes_per_update, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": hbm_frac, "peak_source": hbm_src, "algorithmic_bytes_per_update": bytes_per_update,
+                     "alu_frac": alu_frac, "alu_peak_Tinstr_s": alu_peak, "fp_instr_per_update": 5,
+                     "traffic": None, "traffic_source": "profiles/r2_ncu_2d_warp.md: 1.27 GB of DRAM traffic per half-cycle at 8192^2 fp64 = 4.7 B per update, 1.34 x the algorithmic 3.5 B"},
+        "cpu_baseline": cpu,
         "classic_roofline": {"bound": "hbm", "algorithmic_bytes_per_update": 2 * es, "achieved_GBps": res["classic"] * 2 * es, "peak_GBps": hbm_peak,
                              "frac": res["classic"] * 2 * es / hbm_peak},
         # swept: per half-cycle of L = W/2 timesteps the two launches (bridges, octahedra) each read both arrays over every tile

@@ -57,6 +57,11 @@ int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int tile_width, v
 /* The classic decomposition: one kernel per timestep over all nx*ny points, ping-pong with the workspace. */
 int naive2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, void *cuda_stream);
 
+/* End-to-end convenience used for the `e2e` measurement: copy h_u (HOST, [ny][nx], ideally pinned) to an internal device buffer
+ * (allocated on first use), swept2d_run (use_swept != 0) or naive2d_run on it, copy the result back into h_u, and synchronise
+ * the stream.  Errors as the run calls, SWEPT_ENOMEM. */
+int swept2d_run_host(swept2d_handle_t h, void *h_u, int64_t nsteps, int tile_width, int use_swept, void *cuda_stream);
+
 /* SWEPT2D_OPT_KERNEL: which kernels run tiles of W = 32 (W = 8, 16 always run on the shared-memory kernels).
  *   SWEPT2D_KERNEL_WARP (default)  one warp per tile, both planes of the tile in registers, no barrier; a lane holds two columns of 16
  *                                  rows (the tile's upper half folded onto lanes 16..31): one shuffle per point

@@ -35,7 +35,7 @@ SYMBOLS = (
     "swept_band_layout", "swept_band_owner", "swept_problem_info", "swept_measure_smem_peak", "swept_measure_latencies",
     "swept_run_static", "swept_check",
     # include/swept2d.h
-    "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy",
+    "swept2d_create", "swept2d_run", "naive2d_run", "swept2d_set_option", "swept2d_get_info", "swept2d_destroy", "swept2d_run_host",
 )
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -121,6 +121,7 @@ def lib() -> ctypes.CDLL:
     L.swept2d_create.argtypes = [ctypes.POINTER(vp), i64, i64, dbl, dbl, ctypes.POINTER(_Params2D)]
     L.swept2d_run.argtypes = [vp, vp, i64, ci, vp]
     L.naive2d_run.argtypes = [vp, vp, i64, vp]
+    L.swept2d_run_host.argtypes = [vp, vp, i64, ci, ci, vp]
     L.swept2d_set_option.argtypes = [vp, ci, ci]
     L.swept2d_get_info.argtypes = [vp, ctypes.POINTER(_Info2D)]
     L.swept2d_destroy.argtypes = [vp]
@@ -276,6 +277,20 @@ class Solver2D:
 
     def naive_run(self, u, nsteps: int, stream=None) -> None:
         _check(lib().naive2d_run(self._h, self._ptr(u), int(nsteps), _stream_ptr(stream)))
+
+    def run_host(self, h_u, nsteps: int, tile_width: int = 0, use_swept: bool = True, stream=None) -> None:
+        """h_u: contiguous CPU torch tensor or numpy array [ny, nx] of the handle's dtype (pinned is best); updated in place."""
+        import numpy as np
+        import torch
+        if isinstance(h_u, torch.Tensor) and not h_u.is_cuda and h_u.is_contiguous():
+            ptr, n, es = h_u.data_ptr(), h_u.numel(), h_u.element_size()
+        elif isinstance(h_u, np.ndarray) and h_u.flags["C_CONTIGUOUS"]:
+            ptr, n, es = h_u.ctypes.data, h_u.size, h_u.itemsize
+        else:
+            raise SweptError(EINVAL, "h_u must be a contiguous CPU tensor or numpy array")
+        if n != self.nx * self.ny or es != (8 if self.dtype == F64 else 4):
+            raise SweptError(EINVAL, "h_u has the wrong size or dtype")
+        _check(lib().swept2d_run_host(self._h, ptr, int(nsteps), int(tile_width), 1 if use_swept else 0, _stream_ptr(stream)))
 
     def set_option(self, option: int, value: int) -> None:
         _check(lib().swept2d_set_option(self._h, int(option), int(value)))

@@ -26,6 +26,7 @@ struct swept2d_ctx {
     double dx, dt, alpha;
     ConstBlock cb;
     void *work;
+    void *host_stage;      // device buffer of swept2d_run_host (allocated on first use)
     size_t field_bytes;
     int64_t launches_last, launches_total;
 };
@@ -469,6 +470,7 @@ extern "C" int swept2d_create(swept2d_handle_t *out, int64_t nx, int64_t ny, dou
     if (!h) return swept_fail(SWEPT_ENOMEM, "swept2d_create: out of host memory");
     h->dtype = dtype; h->device = dev; h->kernel = SWEPT2D_KERNEL_WARP; h->nx = nx; h->ny = ny; h->dx = dx; h->dt = dt; h->alpha = alpha;
     h->launches_last = h->launches_total = 0;
+    h->host_stage = nullptr;
     const double Fo = alpha * dt / (dx * dx);                     // row A0: constants on the host in double, cast once
     memset(h->cb.bytes, 0, sizeof h->cb.bytes);
     if (dtype == SWEPT_F64) { Heat2D<double>::Consts c{Fo, 1.0 - 4.0 * Fo}; memcpy(h->cb.bytes, &c, sizeof c); }
@@ -524,6 +526,27 @@ extern "C" int swept2d_run(swept2d_handle_t h, void *d_u, int64_t nsteps, int ti
     return SWEPT_OK;
 }
 
+// End-to-end convenience (the `e2e` measurement of bench.py --heat2d): host buffer in, host buffer out.
+extern "C" int swept2d_run_host(swept2d_handle_t h, void *h_u, int64_t nsteps, int tile_width, int use_swept, void *cuda_stream) {
+    if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_run_host: NULL handle");
+    if (!h_u) return swept_fail(SWEPT_EINVAL, "swept2d_run_host: h_u is NULL");
+    if (nsteps < 0) return swept_fail(SWEPT_EINVAL, "swept2d_run_host: nsteps < 0");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (!h->host_stage) {
+        e = cudaMalloc(&h->host_stage, h->field_bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); h->host_stage = nullptr; return swept_fail(SWEPT_ENOMEM, "swept2d_run_host: cudaMalloc: %s", cudaGetErrorString(e)); }
+    }
+    e = cudaMemcpyAsync(h->host_stage, h_u, h->field_bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return swept_fail(SWEPT_ECUDA, "swept2d_run_host: H2D: %s", cudaGetErrorString(e)); }
+    const int rc = use_swept ? swept2d_run(h, h->host_stage, nsteps, tile_width, cuda_stream) : naive2d_run(h, h->host_stage, nsteps, cuda_stream);
+    if (rc) return rc;
+    e = cudaMemcpyAsync(h_u, h->host_stage, h->field_bytes, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaGetLastError(); return swept_fail(SWEPT_ECUDA, "swept2d_run_host: D2H: %s", cudaGetErrorString(e)); }
+    return SWEPT_OK;
+}
+
 extern "C" int swept2d_set_option(swept2d_handle_t h, int option, int value) {
     if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_set_option: NULL handle");
     if (option != SWEPT2D_OPT_KERNEL || (value != SWEPT2D_KERNEL_WARP && value != SWEPT2D_KERNEL_SMEM && value != SWEPT2D_KERNEL_COLUMN))
@@ -543,6 +566,7 @@ extern "C" int swept2d_get_info(swept2d_handle_t h, swept2d_info_t *info) {
 extern "C" int swept2d_destroy(swept2d_handle_t h) {
     if (!h) return swept_fail(SWEPT_EINVAL, "swept2d_destroy: NULL handle");
     if (h->work) cudaFree(h->work);
+    if (h->host_stage) cudaFree(h->host_stage);
     delete h;
     return SWEPT_OK;
 }

@@ -114,6 +114,22 @@ def test_skinny_2d_grid_at_the_row_limit():
         sw.Solver2D(8, 1 << 19, 1.0, 0.1)
 
 
+def test_run_host_2d_equals_the_device_path():
+    nx, ny, nsteps = 256, 128, 37
+    u0 = wl.heat2d_field(nx, ny)
+    want, _ = _run(nx, ny, np.float64, nsteps, 32, u0=u0)
+    dx, dt = wl.heat2d_grid(max(nx, ny), 0.2)
+    with sw.Solver2D(nx, ny, dx, dt) as s:
+        h = u0.copy()
+        s.run_host(h, nsteps, 32)
+        assert_bits_equal(h, want, "swept2d_run_host, swept")
+        h = u0.copy()
+        s.run_host(h, nsteps, use_swept=False)
+        assert_bits_equal(h, want, "swept2d_run_host, classic")
+        with pytest.raises(sw.SweptError):
+            s.run_host(u0[:64].copy(), nsteps)
+
+
 def test_the_two_2d_kernels_agree():
     """The register kernel and the shared-memory kernel run the same regions in the same tier order with the same store rule:
     identical fields after 1, 2 and 3 half-cycles (odd and even closing alignment)."""
