@@ -86,11 +86,11 @@ enum {
     SWEPT_OPT_INJECT_ABORT = 8,   /* fault injection for tests of the error path (value 1; waits for the handle's work): marks the
                                      handle as if a bounded wait of a launch-free kernel had given up.  The next sweep's waiting
                                      warps leave early, and the mark is reported as described under "Conventions"            */
-    SWEPT_OPT_PACK = 6,           /* heat fp32 on the streaming band kernel: 2 = every warp slot advances TWO bands (half a domain
+    SWEPT_OPT_PACK = 6,           /* heat and KS fp32 on the streaming band kernel: 2 = every warp slot advances TWO bands (half a domain
                                      apart) in lock step on packed f32x2 arithmetic (FADD2 / FMUL2 / FFMA2: half the FP
                                      instructions, per-component IEEE rounding, so the result is bit-identical); 1 = one band
-                                     per slot; 0 (default) = swept_tune's measurement for the tuned width, else on when every
-                                     SM gets at least sixteen bands                                                   */
+                                     per slot; 0 (default) = swept_tune's measurement for the tuned width, else (heat only) on
+                                     when every SM gets at least sixteen bands.  Ignored for fp64 and for Euler      */
     SWEPT_OPT_CHAIN = 5           /* WAVE kernels, launch-free sweep (beyond the paper; removes PAPER.md:232's launch / wave
                                      costs): ONE persistent launch runs all half-cycles of a swept_run.
                                      3 (default) = streaming bands with a communication warp per block: as 2, but the edge
@@ -157,7 +157,7 @@ typedef struct {
     int tuned_blocks_per_sm;     /* resident-blocks cap swept_tune measured as fastest for tuned_tile_width when called with
                                     blocks_per_sm_cap = 0 (0 = none); used while SWEPT_OPT_BLOCKS_PER_SM is 0          */
     int tuned_pack;              /* SWEPT_OPT_PACK value (1 | 2) swept_tune measured as faster for the tuned width and kernel;
-                                    0 = not measured (not heat fp32 on the band kernel)                              */
+                                    0 = not measured (not heat / KS fp32 on the band kernel)                              */
     int tuned_kernel;            /* -1, or SWEPT_KERNEL_SMEM where swept_tune -- under the default options -- measured the
                                     paper-style shared-memory kernels as fastest: swept_run then runs the tuned width on them
                                     (tuned_chain = 0).  Small Euler grids.                                           */

@@ -459,9 +459,10 @@ static int effective_chain(const swept_ctx *h, int W) {
 // Packed pairs of bands (heat fp32, band kernel): the option if set (1 = off, 2 = on); with 0 (auto) the tuner's measurement for the
 // tuned width, else on where every SM gets at least sixteen bands (enough pairs to fill its warps).
 static int effective_pack(const swept_ctx *h, int W) {
-    if (h->problem != SWEPT_HEAT || h->dtype != SWEPT_F32) return 0;
+    if (h->problem == SWEPT_EULER || h->dtype != SWEPT_F32) return 0;
     if (h->pack) return h->pack == 2;
     if (h->tuned_pack && W == h->tuned_tile_width) return h->tuned_pack == 2;
+    if (h->problem == SWEPT_KS) return 0;                            // KS: packed pairs only on request or by the tuner's measurement
     return h->nx / W >= (int64_t)16 * h->sm_count;
 }
 
@@ -598,8 +599,8 @@ extern "C" int swept_tune(swept_handle_t h, void *d_u_scratch, int blocks_per_sm
             for (int ci = 0; ci < ncaps && e == cudaSuccess; ++ci) {
                 const int cap = ncaps == 1 ? blocks_per_sm_cap : caps_auto[ci];
                 h->blocks_per_sm = cap;
-                // heat fp32 on the band kernel: one band per warp slot, and packed pairs
-                const int npack = (saved_pack == 0 && mode == 2 && wave && h->problem == SWEPT_HEAT && h->dtype == SWEPT_F32) ? 2 : 1;
+                // heat and KS fp32 on the band kernel: one band per warp slot, and packed pairs
+                const int npack = (saved_pack == 0 && mode == 2 && wave && h->problem != SWEPT_EULER && h->dtype == SWEPT_F32) ? 2 : 1;
                 for (int pi = 0; pi < npack && e == cudaSuccess; ++pi) {
                     if (npack == 2) h->pack = 1 + pi;
                     float ms_min = 1e30f;

@@ -44,7 +44,7 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
 // Streaming band kernel (swept_band.cuh): ONE launch runs q half-cycles with every band's columns resident in registers /
 // shared memory; `sync` = prog[nx/W] counters (zeroed by the helper).  cudaErrorNotSupported if the schedule does not fit
 // the device (the caller then uses launch_swept_chain).  max_warps > 0 caps the resident warps per SM.
-// pack != 0 (heat fp32 only): two bands per warp slot, advanced by packed f32x2 arithmetic (stencils.cuh float2p).
+// pack != 0 (heat and KS fp32 only): two bands per warp slot, advanced by packed f32x2 arithmetic (stencils.cuh float2p).
 // rt > 0: the remainder tiers as a truncated closing cycle inside the launch (as launch_swept_ring).
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,
                               int sm_count, int max_smem, int max_warps, int pack, cudaStream_t st);

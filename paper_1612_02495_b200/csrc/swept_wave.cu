@@ -50,7 +50,7 @@ cudaError_t launch_swept_chain(int problem, int dtype, void *u, void *w, int64_t
 cudaError_t launch_swept_band(int problem, int dtype, void *u, void *w, int64_t nx, int W, int64_t q, int rt, void *sync, const ConstBlock &cb,
                               int sm_count, int max_smem, int max_warps, int pack, cudaStream_t st) {
     if (problem == SWEPT_HEAT) return launch_swept_band_heat(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, pack, st);
-    if (problem == SWEPT_KS) return launch_swept_band_ks(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, 0, st);
+    if (problem == SWEPT_KS) return launch_swept_band_ks(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, pack, st);
     return launch_swept_band_euler(dtype, u, w, nx, W, q, rt, sync, cb, sm_count, max_smem, max_warps, 0, st);
 }
 

@@ -624,6 +624,35 @@ def test_packed_band_pairs_equal_classic(nx, W, q):
     assert_bits_equal(got, run_swept(w, np.float32, nsteps, W, BAND_V, opts={sw.OPT_PACK: sw.PACK_OFF}), "packed vs one band per slot")
 
 
+@pytest.mark.parametrize("nx,W,q,r", [
+    (1 << 10, 256, 5, 0),             # four bands = two slots (KS band tiles start at W = 256: 64 iterations per tile)
+    (1 << 12, 256, 1, 3),             # q = 1 + a remainder (truncated closing cycle)
+    (1 << 16, 256, 9, 17),
+    (1 << 20, 512, 4, 63),
+    (1 << 22, 1024, 3, 100),          # the config-5 size: 2048 slots
+    (1 << 22, 256, 3, 5),             # 8192 slots: several per warp, parked pairs
+    (1 << 12, 256, 0, 15),            # q = 0: only the truncated cycle
+])
+def test_packed_band_pairs_ks_equal_classic(nx, W, q, r):
+    """KS fp32 on packed f32x2 arithmetic (two sub-timesteps per timestep, radius 2, immediate and negated operands): same bits."""
+    import torch
+    w = _noise(wl.KS, nx)
+    nsteps = q * _sph(wl.KS, W) + r
+    with solver_for(w, np.float32) as s:
+        s.set_option(sw.OPT_CHAIN, sw.CHAIN_BANDS)
+        s.set_option(sw.OPT_PACK, sw.PACK_ON)
+        u = to_dev(w.initial(np.float32))
+        s.swept_run(u, nsteps, W)
+        torch.cuda.synchronize()
+        info = s.info()
+        assert info["last_sweep_launch"] == sw.LAUNCH_BAND and info["launches_last_call"] == 1
+        got = u.cpu().numpy()
+    assert_bits_equal(got, run_naive(w, np.float32, nsteps), f"KS packed band pairs nx={nx} W={W} q={q} r={r}")
+    assert_bits_equal(got, run_swept(w, np.float32, nsteps, W, BAND_V, opts={sw.OPT_PACK: sw.PACK_OFF}), "packed vs one band per slot")
+    if nx <= 1 << 16:
+        assert_bits_equal(got, run_oracle(w, np.float32, nsteps), "KS packed pairs vs oracle")
+
+
 @pytest.mark.parametrize("problem,dtype,nx,W,q,r,pack", [
     (wl.HEAT, np.float64, 1 << 11, 128, 5, 37, 0),       # odd remainder
     (wl.HEAT, np.float64, 1 << 12, 128, 0, 63, 0),       # q = 0: only the truncated cycle, remainder L - 1
