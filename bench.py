@@ -424,10 +424,14 @@ def run_stress(args):
                 s.set_option(sw.OPT_NAIVE_GRAPH, 1)
                 naive = nx * ns_naive / timed(lambda: s.naive_run(u, ns_naive)) / 1e9
                 res = {}
-                for kname, kid, chain, caps in (("ring", sw.KERNEL_WAVE, 3, (0,)), ("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0, 1, 2, 3, 4)),
-                                                ("smem", sw.KERNEL_SMEM, 0, (0, 1, 2, 3, 4))):
+                variants = [("ring", sw.KERNEL_WAVE, 3, (0,)), ("band", sw.KERNEL_WAVE, 2, (0,)), ("chain", sw.KERNEL_WAVE, 1, (0, 1, 2, 3, 4)),
+                            ("smem", sw.KERNEL_SMEM, 0, (0, 1, 2, 3, 4))]
+                if dname == "f32" and problem in ("heat", "ks"):
+                    variants.insert(2, ("bandpack", sw.KERNEL_WAVE, 2, (0,)))     # the band kernel on packed f32x2 pairs (SWEPT_OPT_PACK = 2); "band" = one band per slot
+                for kname, kid, chain, caps in variants:
                     s.set_option(sw.OPT_KERNEL, kid)
                     s.set_option(sw.OPT_CHAIN, chain)
+                    s.set_option(sw.OPT_PACK, sw.PACK_ON if kname == "bandpack" else sw.PACK_OFF)
                     s.set_option(sw.OPT_SWEPT_GRAPH, 1 if kname == "smem" else 0)
                     for W in (32, 64, 128, 256, 512, 1024, 2048):
                         if not s.tile_width_ok(W):
@@ -445,7 +449,7 @@ def run_stress(args):
                             e0.record(stream); s.swept_run(u, ns, W); e1.record(stream); e1.synchronize()
                             t = e0.elapsed_time(e1) * 1e-3
                             ran = sw.LAUNCH_NAMES.get(s.info()["last_sweep_launch"], "-") if kname != "smem" else "smem"
-                            if kname in ("ring", "band") and ran != kname:
+                            if kname in ("ring", "band", "bandpack") and ran != kname.replace("pack", ""):
                                 continue            # the schedule does not fit: this (W) is another kernel's row
                             res[f"{kname}/W={W}/cap={cap}"] = nx * ns / t / 1e9
                 s.set_option(sw.OPT_BLOCKS_PER_SM, 0)
@@ -463,8 +467,8 @@ def run_stress(args):
             for k, v in r["results"].items():
                 kname, W, cap = k.split("/")
                 f.write(f"{r['problem']},{r['dtype']},{r['nx']},{r['nsteps']},{kname},{W[2:]},{cap[4:]},{v:.4f}\n")
-    print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: ring | band | chain (W, cap) | smem (W, cap) |")
-    print("|---|---|---:|---:|---|---:|---|---|---|---|")
+    print("| problem | dtype | classic (graph) | best swept | config | x classic | best per kernel: ring | band (one band per slot) | band, packed pairs | chain (W, cap) | smem (W, cap) |")
+    print("|---|---|---:|---:|---|---:|---|---|---|---|---|")
     for r in rows:
         def bk(k):
             c = {n: v for n, v in r["results"].items() if n.startswith(k + "/")}
@@ -473,7 +477,7 @@ def run_stress(args):
             b = max(c, key=c.get)
             return f"{c[b]:.1f} ({b.split('/', 1)[1]})"
         print(f"| {r['problem']} | {r['dtype']} | {r['classic_graph']:.1f} | {r['best_value']:.1f} | {r['best']} | {r['best_value'] / r['classic_graph']:.1f}x | "
-              f"{bk('ring')} | {bk('band')} | {bk('chain')} | {bk('smem')} |")
+              f"{bk('ring')} | {bk('band')} | {bk('bandpack')} | {bk('chain')} | {bk('smem')} |")
 
 
 def run_heat2d(args):
